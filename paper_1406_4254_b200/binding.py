@@ -1,0 +1,217 @@
+"""Thin Python binding of the C ABI in include/etics.h (argument marshalling only).
+
+Every function has the name of the C entry point it calls; all arithmetic of the method runs in the CUDA
+kernels behind that call.  PyTorch is used for device memory and streams only.  There is no CPU fallback: if
+`libetics.so` is missing or cannot be loaded, `lib()` raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libetics.so")
+
+ETICS_OK = 0
+ETICS_ERR_ARG, ETICS_ERR_LIMIT, ETICS_ERR_ALIGN, ETICS_ERR_WORKSPACE, ETICS_ERR_CUDA = -1, -2, -3, -4, -5
+ETICS_MAX_LMAX, ETICS_MAX_NMAX = 10, 32
+ETICS_WS_SCF_COEFFS, ETICS_WS_SCF_FORCE, ETICS_WS_MEX_FORCE = 0, 1, 2
+
+# every symbol include/etics.h declares (tests check that the library exports all of them)
+EXPORTS = [
+    "etics_status_string", "etics_init", "etics_workspace_bytes", "etics_scf_coeffs", "etics_scf_force",
+    "etics_mex_force", "etics_mex_sort", "etics_host_scratch_bytes", "etics_scf_full_host",
+    "etics_mex_full_host", "etics_probe_dfma", "etics_probe_copy",
+]
+
+_lib = None
+_vp, _ll, _i, _sz = C.c_void_p, C.c_longlong, C.c_int, C.c_size_t
+
+
+class EticsError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {status_string(status)} ({status})")
+
+
+def lib() -> C.CDLL:
+    """Load libetics.so (built by paper_1406_4254_b200.build); fails loudly if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise FileNotFoundError(
+            f"{LIB_PATH} not found: build it with `python -m paper_1406_4254_b200.build` "
+            "(there is no CPU fallback for the ETICS hot path)")
+    L = C.CDLL(LIB_PATH)
+    L.etics_status_string.restype = C.c_char_p
+    L.etics_status_string.argtypes = [_i]
+    L.etics_init.restype = _i
+    L.etics_init.argtypes = []
+    L.etics_workspace_bytes.restype = _sz
+    L.etics_workspace_bytes.argtypes = [_i, _ll, _i, _i]
+    L.etics_scf_coeffs.restype = _i
+    L.etics_scf_coeffs.argtypes = [_vp, _vp, _ll, _i, _i, _vp, _vp, _vp, _sz, _vp]
+    L.etics_scf_force.restype = _i
+    L.etics_scf_force.argtypes = [_vp, _ll, _i, _i, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+    L.etics_mex_force.restype = _i
+    L.etics_mex_force.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _vp, _sz, _vp]
+    L.etics_mex_sort.restype = _i
+    L.etics_mex_sort.argtypes = [_vp, _ll, _vp, _vp, _vp, _sz, _vp]
+    L.etics_host_scratch_bytes.restype = _sz
+    L.etics_host_scratch_bytes.argtypes = [_i, _ll, _i, _i]
+    L.etics_scf_full_host.restype = _i
+    L.etics_scf_full_host.argtypes = [_vp, _vp, _ll, _i, _i, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
+    L.etics_mex_full_host.restype = _i
+    L.etics_mex_full_host.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _vp, _sz, _vp]
+    L.etics_probe_dfma.restype = _i
+    L.etics_probe_dfma.argtypes = [_i, _vp, C.POINTER(C.c_double), _vp]
+    L.etics_probe_copy.restype = _i
+    L.etics_probe_copy.argtypes = [_vp, _vp, _sz, _vp]
+    _lib = L
+    return L
+
+
+def status_string(status: int) -> str:
+    return lib().etics_status_string(status).decode()
+
+
+def num_lm(lmax: int) -> int:
+    return (lmax + 1) * (lmax + 2) // 2
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _dev(t: torch.Tensor, name: str, dtype=torch.float64) -> int:
+    if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise TypeError(f"{name}: expected a contiguous CUDA tensor of dtype {dtype}")
+    return t.data_ptr()
+
+
+def _check(status: int, where: str) -> None:
+    if status != ETICS_OK:
+        raise EticsError(status, where)
+
+
+def etics_init() -> None:
+    _check(lib().etics_init(), "etics_init")
+
+
+def etics_workspace_bytes(which: int, N: int, nmax: int, lmax: int) -> int:
+    return lib().etics_workspace_bytes(which, N, nmax, lmax)
+
+
+def _workspace(which: int, N: int, nmax: int, lmax: int, device, workspace):
+    need = etics_workspace_bytes(which, N, nmax, lmax)
+    if workspace is None:
+        workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=device)
+    return workspace, workspace.numel() * workspace.element_size()
+
+
+def etics_scf_coeffs(pos, mass, nmax: int, lmax: int, A=None, B=None, workspace=None, stream=None):
+    """pos (3,N), mass (N,) CUDA fp64 -> A, B (T,) CUDA fp64.  See include/etics.h."""
+    N = mass.shape[0]
+    T = (nmax + 1) * num_lm(lmax)
+    if A is None:
+        A = torch.empty(T, dtype=torch.float64, device=pos.device)
+    if B is None:
+        B = torch.empty(T, dtype=torch.float64, device=pos.device)
+    workspace, wsb = _workspace(ETICS_WS_SCF_COEFFS, N, nmax, lmax, pos.device, workspace)
+    assert pos.shape == (3, N) and A.shape == (T,) and B.shape == (T,)
+    s = lib().etics_scf_coeffs(_dev(pos, "pos"), _dev(mass, "mass"), N, nmax, lmax, _dev(A, "A"), _dev(B, "B"),
+                               workspace.data_ptr(), wsb, _stream(stream))
+    _check(s, "etics_scf_coeffs")
+    return A, B
+
+
+def etics_scf_force(pos, nmax: int, lmax: int, A, B, acc=None, pot=None, stream=None):
+    """pos (3,N), A, B (T,) CUDA fp64 -> acc (3,N), pot (N,)."""
+    N = pos.shape[1]
+    T = (nmax + 1) * num_lm(lmax)
+    if acc is None:
+        acc = torch.empty((3, N), dtype=torch.float64, device=pos.device)
+    if pot is None:
+        pot = torch.empty(N, dtype=torch.float64, device=pos.device)
+    assert pos.shape == (3, N) and A.shape == (T,) and B.shape == (T,) and acc.shape == (3, N) and pot.shape == (N,)
+    s = lib().etics_scf_force(_dev(pos, "pos"), N, nmax, lmax, _dev(A, "A"), _dev(B, "B"), _dev(acc, "acc"),
+                              _dev(pot, "pot"), None, 0, _stream(stream))
+    _check(s, "etics_scf_force")
+    return acc, pot
+
+
+def etics_mex_force(pos, mass, lmax: int, acc=None, pot=None, workspace=None, stream=None):
+    """pos (3,N), mass (N,) CUDA fp64 -> acc (3,N), pot (N,) at the particles' original indices."""
+    N = mass.shape[0]
+    if acc is None:
+        acc = torch.empty((3, N), dtype=torch.float64, device=pos.device)
+    if pot is None:
+        pot = torch.empty(N, dtype=torch.float64, device=pos.device)
+    workspace, wsb = _workspace(ETICS_WS_MEX_FORCE, N, 0, lmax, pos.device, workspace)
+    assert pos.shape == (3, N) and acc.shape == (3, N) and pot.shape == (N,)
+    s = lib().etics_mex_force(_dev(pos, "pos"), _dev(mass, "mass"), N, lmax, _dev(acc, "acc"), _dev(pot, "pot"),
+                              workspace.data_ptr(), wsb, _stream(stream))
+    _check(s, "etics_mex_force")
+    return acc, pot
+
+
+def etics_mex_sort(pos, keys_sorted=None, perm=None, workspace=None, stream=None):
+    """pos (3,N) CUDA fp64 -> keys_sorted (N,) int64 holding the uint64 bit patterns, perm (N,) int32 holding uint32."""
+    N = pos.shape[1]
+    if keys_sorted is None:
+        keys_sorted = torch.empty(N, dtype=torch.int64, device=pos.device)
+    if perm is None:
+        perm = torch.empty(N, dtype=torch.int32, device=pos.device)
+    workspace, wsb = _workspace(ETICS_WS_MEX_FORCE, N, 0, 0, pos.device, workspace)
+    s = lib().etics_mex_sort(_dev(pos, "pos"), N, _dev(keys_sorted, "keys_sorted", torch.int64),
+                             _dev(perm, "perm", torch.int32), workspace.data_ptr(), wsb, _stream(stream))
+    _check(s, "etics_mex_sort")
+    return keys_sorted, perm
+
+
+def etics_host_scratch_bytes(method: int, N: int, nmax: int, lmax: int) -> int:
+    return lib().etics_host_scratch_bytes(method, N, nmax, lmax)
+
+
+def _host(t: torch.Tensor, name: str) -> int:
+    if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise TypeError(f"{name}: expected a contiguous CPU float64 tensor")
+    return t.data_ptr()
+
+
+def etics_scf_full_host(pos_h, mass_h, nmax: int, lmax: int, acc_h, pot_h, scratch, A_h=None, B_h=None, stream=None):
+    """Host buffers in/out (pinned recommended); `scratch` is a CUDA uint8 tensor of etics_host_scratch_bytes(0,...)."""
+    N = mass_h.shape[0]
+    s = lib().etics_scf_full_host(_host(pos_h, "pos_h"), _host(mass_h, "mass_h"), N, nmax, lmax,
+                                  None if A_h is None else _host(A_h, "A_h"), None if B_h is None else _host(B_h, "B_h"),
+                                  _host(acc_h, "acc_h"), _host(pot_h, "pot_h"),
+                                  scratch.data_ptr(), scratch.numel() * scratch.element_size(), _stream(stream))
+    _check(s, "etics_scf_full_host")
+
+
+def etics_mex_full_host(pos_h, mass_h, lmax: int, acc_h, pot_h, scratch, stream=None):
+    N = mass_h.shape[0]
+    s = lib().etics_mex_full_host(_host(pos_h, "pos_h"), _host(mass_h, "mass_h"), N, lmax,
+                                  _host(acc_h, "acc_h"), _host(pot_h, "pot_h"),
+                                  scratch.data_ptr(), scratch.numel() * scratch.element_size(), _stream(stream))
+    _check(s, "etics_mex_full_host")
+
+
+def etics_probe_dfma(iters: int, sink, stream=None) -> float:
+    """Enqueue the fp64-FMA probe; returns the number of floating-point operations it performs."""
+    flops = C.c_double(0.0)
+    s = lib().etics_probe_dfma(iters, _dev(sink, "sink"), C.byref(flops), _stream(stream))
+    _check(s, "etics_probe_dfma")
+    return flops.value
+
+
+def etics_probe_copy(dst, src, stream=None) -> int:
+    nbytes = src.numel() * src.element_size()
+    s = lib().etics_probe_copy(dst.data_ptr(), src.data_ptr(), nbytes, _stream(stream))
+    _check(s, "etics_probe_copy")
+    return 2 * nbytes

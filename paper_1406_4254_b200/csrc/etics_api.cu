@@ -1,0 +1,176 @@
+// etics_api.cu — the C ABI of include/etics.h: argument checks, workspace sizes, launch sequences.
+// Nothing here computes; every step of the path runs in the kernels of scf.cu / mex.cu.
+#include "etics_common.cuh"
+
+using namespace etics;
+
+namespace {
+
+inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+etics_status check_sizes(long long N, int nmax, int lmax) {
+    if (N < 1 || N >= (1LL << 31) || nmax < 0 || lmax < 0) return ETICS_ERR_ARG;
+    if (nmax > ETICS_MAX_NMAX || lmax > ETICS_MAX_LMAX) return ETICS_ERR_LIMIT;
+    return ETICS_OK;
+}
+
+inline etics_status from_cuda(cudaError_t e) { return e == cudaSuccess ? ETICS_OK : ETICS_ERR_CUDA; }
+
+}  // namespace
+
+extern "C" {
+
+const char* etics_status_string(etics_status s) {
+    switch (s) {
+        case ETICS_OK: return "ETICS_OK";
+        case ETICS_ERR_ARG: return "ETICS_ERR_ARG: invalid argument (N, nmax, lmax, null pointer or selector)";
+        case ETICS_ERR_LIMIT: return "ETICS_ERR_LIMIT: nmax or lmax beyond ETICS_MAX_NMAX / ETICS_MAX_LMAX";
+        case ETICS_ERR_ALIGN: return "ETICS_ERR_ALIGN: pointer not 16-byte aligned";
+        case ETICS_ERR_WORKSPACE: return "ETICS_ERR_WORKSPACE: workspace too small";
+        case ETICS_ERR_CUDA: return "ETICS_ERR_CUDA: CUDA runtime or launch error";
+        default: return "ETICS: unknown status";
+    }
+}
+
+etics_status etics_init(void) {
+    cudaError_t e = scf_init_constants();
+    if (e != cudaSuccess) return ETICS_ERR_CUDA;
+    return from_cuda(mex_init_constants());
+}
+
+size_t etics_workspace_bytes(int which, long long N, int nmax, int lmax) {
+    if (which == ETICS_WS_MEX_FORCE) nmax = 0;
+    if (check_sizes(N, nmax, lmax) != ETICS_OK) return 0;
+    size_t b = 0;
+    switch (which) {
+        case ETICS_WS_SCF_COEFFS: b = scf_coeffs_workspace(N, nmax, lmax); break;
+        case ETICS_WS_SCF_FORCE: b = 0; break;
+        case ETICS_WS_MEX_FORCE: b = mex_workspace(N, lmax); break;
+        default: return 0;
+    }
+    return b < 256 ? 256 : round_up(b, 256);
+}
+
+etics_status etics_scf_coeffs(const double* pos, const double* mass, long long N, int nmax, int lmax,
+                              double* A, double* B, void* workspace, size_t workspace_bytes, void* stream) {
+    etics_status s = check_sizes(N, nmax, lmax);
+    if (s != ETICS_OK) return s;
+    if (!pos || !mass || !A || !B || !workspace) return ETICS_ERR_ARG;
+    if (misaligned(pos) || misaligned(mass) || misaligned(A) || misaligned(B) || misaligned(workspace)) return ETICS_ERR_ALIGN;
+    if (workspace_bytes < etics_workspace_bytes(ETICS_WS_SCF_COEFFS, N, nmax, lmax)) return ETICS_ERR_WORKSPACE;
+    return from_cuda(scf_coeffs_launch(pos, mass, N, nmax, lmax, A, B, workspace, static_cast<cudaStream_t>(stream)));
+}
+
+etics_status etics_scf_force(const double* pos, long long N, int nmax, int lmax, const double* A, const double* B,
+                             double* acc, double* pot, void* workspace, size_t workspace_bytes, void* stream) {
+    etics_status s = check_sizes(N, nmax, lmax);
+    if (s != ETICS_OK) return s;
+    (void)workspace; (void)workspace_bytes;   // this call needs no workspace; NULL / 0 are accepted
+    if (!pos || !A || !B || !acc || !pot) return ETICS_ERR_ARG;
+    if (misaligned(pos) || misaligned(A) || misaligned(B) || misaligned(acc) || misaligned(pot)) return ETICS_ERR_ALIGN;
+    return from_cuda(scf_force_launch(pos, N, nmax, lmax, A, B, acc, pot, static_cast<cudaStream_t>(stream)));
+}
+
+etics_status etics_mex_force(const double* pos, const double* mass, long long N, int lmax,
+                             double* acc, double* pot, void* workspace, size_t workspace_bytes, void* stream) {
+    etics_status s = check_sizes(N, 0, lmax);
+    if (s != ETICS_OK) return s;
+    if (!pos || !mass || !acc || !pot || !workspace) return ETICS_ERR_ARG;
+    if (misaligned(pos) || misaligned(mass) || misaligned(acc) || misaligned(pot) || misaligned(workspace)) return ETICS_ERR_ALIGN;
+    if (workspace_bytes < etics_workspace_bytes(ETICS_WS_MEX_FORCE, N, 0, lmax)) return ETICS_ERR_WORKSPACE;
+    return from_cuda(mex_force_launch(pos, mass, N, lmax, acc, pot, workspace, static_cast<cudaStream_t>(stream)));
+}
+
+etics_status etics_mex_sort(const double* pos, long long N, unsigned long long* keys_sorted, unsigned int* perm,
+                            void* workspace, size_t workspace_bytes, void* stream) {
+    etics_status s = check_sizes(N, 0, 0);
+    if (s != ETICS_OK) return s;
+    if (!pos || !keys_sorted || !perm || !workspace) return ETICS_ERR_ARG;
+    if (misaligned(pos) || misaligned(keys_sorted) || misaligned(perm) || misaligned(workspace)) return ETICS_ERR_ALIGN;
+    if (workspace_bytes < etics_workspace_bytes(ETICS_WS_MEX_FORCE, N, 0, 0)) return ETICS_ERR_WORKSPACE;
+    return from_cuda(mex_sort_launch(pos, N, keys_sorted, perm, workspace, static_cast<cudaStream_t>(stream)));
+}
+
+// ---- host-buffer entry points ------------------------------------------------------------------------------
+// Scratch layout: pos[3N] | mass[N] | acc[3N] | pot[N] | A[T] | B[T] | workspace, each 256-byte aligned.
+static size_t seg(size_t doubles) { return round_up(doubles * sizeof(double), 256); }
+
+size_t etics_host_scratch_bytes(int method, long long N, int nmax, int lmax) {
+    if (method != 0 && method != 1) return 0;
+    if (method == 1) nmax = 0;
+    if (check_sizes(N, nmax, lmax) != ETICS_OK) return 0;
+    const size_t T = (size_t)(nmax + 1) * num_lm(lmax);
+    size_t b = seg(3 * (size_t)N) + seg((size_t)N) + seg(3 * (size_t)N) + seg((size_t)N) + 2 * seg(T);
+    b += etics_workspace_bytes(method == 0 ? ETICS_WS_SCF_COEFFS : ETICS_WS_MEX_FORCE, N, nmax, lmax);
+    return b;
+}
+
+etics_status etics_scf_full_host(const double* pos_h, const double* mass_h, long long N, int nmax, int lmax,
+                                 double* A_h, double* B_h, double* acc_h, double* pot_h,
+                                 void* device_scratch, size_t scratch_bytes, void* stream) {
+    etics_status s = check_sizes(N, nmax, lmax);
+    if (s != ETICS_OK) return s;
+    if (!pos_h || !mass_h || !acc_h || !pot_h || !device_scratch) return ETICS_ERR_ARG;
+    if (misaligned(device_scratch)) return ETICS_ERR_ALIGN;
+    if (scratch_bytes < etics_host_scratch_bytes(0, N, nmax, lmax)) return ETICS_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t T = (size_t)(nmax + 1) * num_lm(lmax), n = (size_t)N;
+    char* p = static_cast<char*>(device_scratch);
+    double* d_pos = reinterpret_cast<double*>(p); p += seg(3 * n);
+    double* d_mass = reinterpret_cast<double*>(p); p += seg(n);
+    double* d_acc = reinterpret_cast<double*>(p); p += seg(3 * n);
+    double* d_pot = reinterpret_cast<double*>(p); p += seg(n);
+    double* d_A = reinterpret_cast<double*>(p); p += seg(T);
+    double* d_B = reinterpret_cast<double*>(p); p += seg(T);
+    const size_t wsb = etics_workspace_bytes(ETICS_WS_SCF_COEFFS, N, nmax, lmax);
+    if (cudaMemcpyAsync(d_pos, pos_h, 3 * n * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return ETICS_ERR_CUDA;
+    if (cudaMemcpyAsync(d_mass, mass_h, n * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return ETICS_ERR_CUDA;
+    s = etics_scf_coeffs(d_pos, d_mass, N, nmax, lmax, d_A, d_B, p, wsb, stream);
+    if (s != ETICS_OK) return s;
+    s = etics_scf_force(d_pos, N, nmax, lmax, d_A, d_B, d_acc, d_pot, nullptr, 0, stream);
+    if (s != ETICS_OK) return s;
+    if (cudaMemcpyAsync(acc_h, d_acc, 3 * n * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return ETICS_ERR_CUDA;
+    if (cudaMemcpyAsync(pot_h, d_pot, n * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return ETICS_ERR_CUDA;
+    if (A_h && cudaMemcpyAsync(A_h, d_A, T * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return ETICS_ERR_CUDA;
+    if (B_h && cudaMemcpyAsync(B_h, d_B, T * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return ETICS_ERR_CUDA;
+    return ETICS_OK;
+}
+
+etics_status etics_mex_full_host(const double* pos_h, const double* mass_h, long long N, int lmax,
+                                 double* acc_h, double* pot_h, void* device_scratch, size_t scratch_bytes, void* stream) {
+    etics_status s = check_sizes(N, 0, lmax);
+    if (s != ETICS_OK) return s;
+    if (!pos_h || !mass_h || !acc_h || !pot_h || !device_scratch) return ETICS_ERR_ARG;
+    if (misaligned(device_scratch)) return ETICS_ERR_ALIGN;
+    if (scratch_bytes < etics_host_scratch_bytes(1, N, 0, lmax)) return ETICS_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t T = (size_t)num_lm(lmax), n = (size_t)N;
+    char* p = static_cast<char*>(device_scratch);
+    double* d_pos = reinterpret_cast<double*>(p); p += seg(3 * n);
+    double* d_mass = reinterpret_cast<double*>(p); p += seg(n);
+    double* d_acc = reinterpret_cast<double*>(p); p += seg(3 * n);
+    double* d_pot = reinterpret_cast<double*>(p); p += seg(n);
+    p += 2 * seg(T);
+    const size_t wsb = etics_workspace_bytes(ETICS_WS_MEX_FORCE, N, 0, lmax);
+    if (cudaMemcpyAsync(d_pos, pos_h, 3 * n * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return ETICS_ERR_CUDA;
+    if (cudaMemcpyAsync(d_mass, mass_h, n * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return ETICS_ERR_CUDA;
+    s = etics_mex_force(d_pos, d_mass, N, lmax, d_acc, d_pot, p, wsb, stream);
+    if (s != ETICS_OK) return s;
+    if (cudaMemcpyAsync(acc_h, d_acc, 3 * n * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return ETICS_ERR_CUDA;
+    if (cudaMemcpyAsync(pot_h, d_pot, n * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return ETICS_ERR_CUDA;
+    return ETICS_OK;
+}
+
+// ---- probes ----------------------------------------------------------------------------------------------
+etics_status etics_probe_dfma(int iters, double* sink, double* flops_out, void* stream) {
+    if (iters < 1 || !sink) return ETICS_ERR_ARG;
+    return from_cuda(probe_dfma_launch(iters, sink, flops_out, static_cast<cudaStream_t>(stream)));
+}
+
+etics_status etics_probe_copy(void* dst, const void* src, size_t bytes, void* stream) {
+    if (!dst || !src || bytes < 16) return ETICS_ERR_ARG;
+    if (misaligned(dst) || misaligned(src)) return ETICS_ERR_ALIGN;
+    return from_cuda(probe_copy_launch(dst, src, bytes, static_cast<cudaStream_t>(stream)));
+}
+
+}  // extern "C"
