@@ -1,9 +1,739 @@
-// mex.cu — MEX half of the hot path (placeholder until the kernels land; returns cudaErrorNotSupported).
+// mex.cu — MEX half of the hot path (SURVEY.md §8(a) M1–M7) for sm_100a.
+//
+//   mex_keygen_kernel      M1: key = bits(r^2) (rounding pinned: t=x*x; t=fma(y,y,t); t=fma(z,z,t)), idx = k, and the
+//                          256-bin histograms of all eight key bytes in the same pass.
+//   mex_radix_pass_kernel  M2: one stable LSD pass over 8 key bits, "onesweep" style: each tile ranks its keys with
+//                          warp match/popc, reorders them in shared memory, obtains its global bucket offsets by a
+//                          decoupled lookback over the preceding tiles' per-digit counts (integers: exact, so the
+//                          result does not depend on timing) and writes keys + payload once.  Hand-written, no CUB.
+//   mex_gather_kernel      M3: sorted order -> per-particle geometry records (r, 1/r, cos/sin theta, cos/sin phi, m)
+//                          in a chunk-transposed SoA layout that the scan kernels read fully coalesced.
+//   mex_aggregate_kernel   M4+M5a: every thread owns K consecutive sorted particles and sums their moments
+//                          w_lm m r^l P_lm {cos,sin} m phi and w_lm m r^-(l+1) P_lm {cos,sin} m phi; block-level
+//                          exclusive scan (inside-out for q, outside-in for p) in shared memory; per-chunk prefixes
+//                          and per-tile totals to the workspace.
+//   mex_tilescan_kernel    M5b: exclusive scan of the tile totals (forward for q, backward for p), fixed order.
+//   mex_evaluate_kernel    M5c+M6+M7: each thread re-walks its K particles forwards carrying q and backwards
+//                          carrying p (never "total minus prefix": that cancels catastrophically), accumulates
+//                          potential and spherical force components, transforms to Cartesian and scatters to the
+//                          particle's original index.
+//
+// The fp64 scans use a fixed summation order (thread chunk -> tile -> grid), so results are bitwise reproducible.
+// The (l,m) set is split into groups of whole m-columns (the Legendre l-recurrence runs along a column), so a
+// thread never holds more than ~17 (l,m) pairs of running sums in registers at a time.
+//
+// What the paper did instead (prior art, §3.2): Thrust merge sort of particle structs, a cache
+// kernel, then per l: a summand kernel writing q_lm, p_lm of every particle to global memory, one Thrust
+// exclusive_scan per (m, re/im, direction), a partial-force kernel; finally a coordinate-transform kernel.
 #include "etics_common.cuh"
 
 namespace etics {
-cudaError_t mex_init_constants() { return cudaSuccess; }
-size_t mex_workspace(long long, int) { return 256; }
-cudaError_t mex_sort_launch(const double*, long long, unsigned long long*, unsigned int*, void*, cudaStream_t) { return cudaErrorNotSupported; }
-cudaError_t mex_force_launch(const double*, const double*, long long, int, double*, double*, void*, cudaStream_t) { return cudaErrorNotSupported; }
+
+cudaError_t mex_init_constants() { return cudaSuccess; }   // every MEX constant is a compile-time literal
+
+// =========================================================================================================
+// Column groups.  Column m holds the pairs (l,m), l = m..LMAX.  kGroupOf[LMAX][m] assigns columns to groups of
+// at most 17 pairs, balanced by hand.
+// =========================================================================================================
+__host__ __device__ constexpr int mex_num_groups(int lmax) {
+    return lmax <= 4 ? 1 : lmax <= 6 ? 2 : lmax <= 8 ? 3 : 4;
+}
+__host__ __device__ constexpr int mex_group_of(int lmax, int m) {
+    switch (lmax) {
+        case 5: return m <= 1 ? 0 : 1;                                            // 11 | 10
+        case 6: return (m <= 1 || m == 6) ? 0 : 1;                                // 14 | 14
+        case 7: return (m == 0 || m == 3) ? 0 : (m == 1 || m == 4 || m == 7) ? 1 : 2;   // 13 | 12 | 11
+        case 8: return (m == 0 || m == 3) ? 0 : (m == 1 || m == 2) ? 1 : 2;       // 15 | 15 | 15
+        case 9: return (m == 0 || m == 6) ? 0 : (m == 1 || m == 5) ? 1 : (m == 2 || m == 4) ? 2 : 3;   // 14 14 14 13
+        case 10: return (m == 0 || m == 5) ? 0 : (m == 1 || m == 4) ? 1 : (m == 2 || m == 3) ? 2 : 3;  // 17 17 17 15
+        default: return 0;
+    }
+}
+// running sums per direction of column m: cos only for m = 0, (cos, sin) otherwise
+__host__ __device__ constexpr int mex_col_slots(int lmax, int m) { return (lmax - m + 1) * (m == 0 ? 1 : 2); }
+// first slot of column m inside its group
+__host__ __device__ constexpr int mex_slot_base(int lmax, int m) {
+    int s = 0;
+    for (int mm = 0; mm < m; ++mm)
+        if (mex_group_of(lmax, mm) == mex_group_of(lmax, m)) s += mex_col_slots(lmax, mm);
+    return s;
+}
+__host__ __device__ constexpr int mex_group_slots(int lmax, int g) {
+    int s = 0;
+    for (int m = 0; m <= lmax; ++m)
+        if (mex_group_of(lmax, m) == g) s += mex_col_slots(lmax, m);
+    return s;
+}
+// first global row of group g; rows of a group: [0,NS) = q slots (forward), [NS,2NS) = p slots (backward)
+__host__ __device__ constexpr int mex_row_base(int lmax, int g) {
+    int s = 0;
+    for (int gg = 0; gg < g; ++gg) s += 2 * mex_group_slots(lmax, gg);
+    return s;
+}
+__host__ __device__ constexpr int mex_total_rows(int lmax) { return mex_row_base(lmax, mex_num_groups(lmax)); }
+__host__ __device__ constexpr int mex_max_group_slots(int lmax) {
+    int s = 0;
+    for (int g = 0; g < mex_num_groups(lmax); ++g) s = mex_group_slots(lmax, g) > s ? mex_group_slots(lmax, g) : s;
+    return s;
+}
+// w_lm = (2 - delta_m0) (l-m)!/(l+m)!   (eq. 15's 4 pi/(2l+1) times the orthonormal Y_lm normalisation, +-m folded)
+__host__ __device__ constexpr double mex_w(int l, int m) {
+    double v = (m == 0) ? 1.0 : 2.0;
+    for (int k = l - m + 1; k <= l + m; ++k) v /= double(k);
+    return v;
+}
+__host__ __device__ constexpr double mex_dfact(int m) {   // (2m-1)!!
+    double v = 1.0;
+    for (int k = 1; k <= m; ++k) v *= double(2 * k - 1);
+    return v;
+}
+
+// Tile geometry of the scan kernels: kMexThreads chunks of kMexK consecutive sorted particles.
+constexpr int kMexThreads = 128;
+constexpr int kMexK = 8;
+constexpr int kMexTile = kMexThreads * kMexK;
+constexpr int kRecFields = 8;   // r, 1/r, cos th, sin th, cos ph, sin ph, mass, (spare)
+
+// Radix sort geometry.
+constexpr int kSortThreads = 256;
+constexpr int kSortItems = 16;
+constexpr int kSortTile = kSortThreads * kSortItems;
+constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kSortPasses = 8;
+
+struct MexLayout {
+    long long N;
+    int lmax;
+    long long sort_tiles, tiles, chunks;   // chunks = tiles * kMexThreads
+    int rows;
+    size_t off_zero, zero_bytes;           // [hist 8x256 u32 | tickets 8 u32 | status sort_tiles*256 u64]
+    size_t off_hist, off_ticket, off_status;
+    size_t off_keysA, off_keysB, off_idxA, off_idxB;
+    size_t off_rec, off_idxT, off_pre, off_tot;
+    size_t total;
+};
+
+static MexLayout make_mex_layout(long long N, int lmax) {
+    MexLayout L{};
+    L.N = N; L.lmax = lmax;
+    L.sort_tiles = (N + kSortTile - 1) / kSortTile;
+    L.tiles = (N + kMexTile - 1) / kMexTile;
+    L.chunks = L.tiles * kMexThreads;
+    L.rows = mex_total_rows(lmax);
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o += round_up(bytes, 256); return at; };
+    L.off_zero = o;
+    L.off_hist = take((size_t)kSortPasses * 256 * sizeof(unsigned));
+    L.off_ticket = take(64);
+    L.off_status = take((size_t)L.sort_tiles * 256 * sizeof(unsigned long long));
+    L.zero_bytes = o - L.off_zero;
+    L.off_keysA = take((size_t)N * 8);
+    L.off_keysB = take((size_t)N * 8);
+    L.off_idxA = take((size_t)N * 4);
+    L.off_idxB = take((size_t)N * 4);
+    L.off_rec = take((size_t)L.tiles * kRecFields * kMexTile * 8);
+    L.off_idxT = take((size_t)L.tiles * kMexTile * 4);
+    L.off_pre = take((size_t)L.rows * L.chunks * 8);
+    L.off_tot = take((size_t)L.rows * L.tiles * 8);
+    L.total = o;
+    return L;
+}
+
+size_t mex_workspace(long long N, int lmax) { return make_mex_layout(N, lmax).total; }
+
+// =========================================================================================================
+// M1: keys + byte histograms.
+// =========================================================================================================
+__device__ __forceinline__ unsigned long long mex_key(double x, double y, double z) {
+    double t = __dmul_rn(x, x);
+    t = __fma_rn(y, y, t);
+    t = __fma_rn(z, z, t);
+    return (unsigned long long)__double_as_longlong(t);   // r^2 >= 0: the bit pattern is monotone in r^2
+}
+
+__global__ void __launch_bounds__(256)
+mex_keygen_kernel(const double* __restrict__ pos, long long N, unsigned long long* __restrict__ keys,
+                  unsigned* __restrict__ idx, unsigned* __restrict__ hist) {
+    __shared__ unsigned sh[kSortPasses * 256];
+    for (int i = threadIdx.x; i < kSortPasses * 256; i += blockDim.x) sh[i] = 0;
+    __syncthreads();
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < N; k += stride) {
+        const unsigned long long key = mex_key(pos[k], pos[N + k], pos[2 * N + k]);
+        keys[k] = key;
+        idx[k] = (unsigned)k;
+#pragma unroll
+        for (int p = 0; p < kSortPasses; ++p) atomicAdd(&sh[p * 256 + (unsigned)((key >> (8 * p)) & 255u)], 1u);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < kSortPasses * 256; i += blockDim.x)
+        if (sh[i]) atomicAdd(&hist[i], sh[i]);
+}
+
+// =========================================================================================================
+// M2: one stable LSD radix pass (8 bits) with decoupled lookback.
+// status word: [63:56] tag (2*pass+1 = tile aggregate, 2*pass+2 = inclusive prefix, anything else = not yet),
+//              [55:0] count.  The buffer is zeroed once per sort; tags of earlier passes read as "not yet".
+// =========================================================================================================
+constexpr unsigned long long kCountMask = (1ull << 56) - 1;
+
+struct SortSmem {
+    unsigned warp_hist[kSortWarps][256];   // per-warp digit counts -> exclusive offsets of the warp inside the tile
+    unsigned local_off[256];               // exclusive digit offsets inside the tile
+    unsigned gbase[256];                   // global position of the tile's first key of digit d, minus local_off[d]
+    unsigned scan_tmp[kSortWarps];
+    unsigned tile;
+    unsigned long long keys[kSortTile];
+    unsigned idx[kSortTile];
+};
+
+__device__ __forceinline__ unsigned block_exclusive_scan_256(unsigned v, unsigned* tmp, unsigned* total) {
+    // kSortThreads == 256 threads, one value each
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    unsigned inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) tmp[warp] = inc;
+    __syncthreads();
+    unsigned woff = 0, tot = 0;
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) {
+        const unsigned t = tmp[w];
+        if (w < warp) woff += t;
+        tot += t;
+    }
+    __syncthreads();
+    if (total) *total = tot;
+    return woff + inc - v;
+}
+
+__global__ void __launch_bounds__(kSortThreads)
+mex_radix_pass_kernel(const unsigned long long* __restrict__ keys_in, const unsigned* __restrict__ idx_in,
+                      unsigned long long* __restrict__ keys_out, unsigned* __restrict__ idx_out,
+                      long long N, int pass, const unsigned* __restrict__ hist, unsigned* __restrict__ tickets,
+                      unsigned long long* status) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    SortSmem& S = *reinterpret_cast<SortSmem*>(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int shift = 8 * pass;
+
+    if (tid == 0) S.tile = atomicAdd(&tickets[pass], 1u);   // tiles are numbered in the order they start running
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) S.warp_hist[w][tid] = 0;
+    __syncthreads();
+    const long long tile = S.tile;
+    const long long base = tile * kSortTile + (long long)warp * (32 * kSortItems);
+
+    // ---- load (warp-striped: item i of the warp's 512-key slice sits at base + 32 i + lane) and rank -----------
+    unsigned long long key[kSortItems];
+    unsigned pay[kSortItems];
+    unsigned short rank[kSortItems];
+#pragma unroll
+    for (int i = 0; i < kSortItems; ++i) {
+        const long long k = base + 32 * i + lane;
+        key[i] = ~0ull;            // padding sorts last in every pass and is never written (position >= N)
+        pay[i] = 0;
+        if (k < N) { key[i] = keys_in[k]; pay[i] = idx_in[k]; }
+    }
+    const unsigned lt_mask = (1u << lane) - 1u;
+    unsigned* wh = S.warp_hist[warp];
+#pragma unroll
+    for (int i = 0; i < kSortItems; ++i) {
+        const unsigned d = (unsigned)(key[i] >> shift) & 255u;
+        const unsigned peers = __match_any_sync(0xffffffffu, d);
+        const int leader = __ffs(peers) - 1;
+        unsigned prior = 0;
+        if (lane == leader) { prior = wh[d]; wh[d] = prior + __popc(peers); }
+        prior = __shfl_sync(0xffffffffu, prior, leader);
+        rank[i] = (unsigned short)(prior + __popc(peers & lt_mask));
+        __syncwarp();
+    }
+    __syncthreads();
+
+    // ---- thread d owns digit d: warp offsets, tile count, lookback ---------------------------------------------
+    unsigned count = 0;
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) {
+        const unsigned t = S.warp_hist[w][tid];
+        S.warp_hist[w][tid] = count;
+        count += t;
+    }
+    const unsigned long long tag_agg = (unsigned long long)(2 * pass + 1) << 56;
+    const unsigned long long tag_inc = (unsigned long long)(2 * pass + 2) << 56;
+    volatile unsigned long long* my_status = status + (size_t)tile * 256 + tid;
+    if (tile > 0) *my_status = tag_agg | count;
+
+    const unsigned loc = block_exclusive_scan_256(count, S.scan_tmp, nullptr);
+    const unsigned hcount = hist[pass * 256 + tid];
+    const unsigned hbase = block_exclusive_scan_256(hcount, S.scan_tmp, nullptr);   // global start of bucket d
+
+    unsigned long long excl = 0;
+    if (tile > 0) {
+        long long t = tile - 1;
+        while (true) {
+            const unsigned long long v = *(volatile unsigned long long*)(status + (size_t)t * 256 + tid);
+            const unsigned long long tag = v & ~kCountMask;
+            if (tag == tag_inc) { excl += v & kCountMask; break; }
+            if (tag == tag_agg) { excl += v & kCountMask; --t; }
+        }
+    }
+    *my_status = tag_inc | (excl + count);
+    S.local_off[tid] = loc;
+    S.gbase[tid] = hbase + (unsigned)excl - loc;
+    __syncthreads();
+
+    // ---- reorder inside the tile (stable), then write runs of equal digits ---------------------------------------
+#pragma unroll
+    for (int i = 0; i < kSortItems; ++i) {
+        const unsigned d = (unsigned)(key[i] >> shift) & 255u;
+        const unsigned p = S.local_off[d] + wh[d] + rank[i];
+        S.keys[p] = key[i];
+        S.idx[p] = pay[i];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < kSortItems; ++i) {
+        const unsigned j = i * kSortThreads + tid;
+        const unsigned long long kk = S.keys[j];
+        const unsigned d = (unsigned)(kk >> shift) & 255u;
+        const unsigned g = S.gbase[d] + j;
+        if ((long long)g < N) { keys_out[g] = kk; idx_out[g] = S.idx[j]; }
+    }
+}
+
+// =========================================================================================================
+// M3: gather into geometry records.  Record of the particle at sorted position p = tile*TP + c*K + k
+// (chunk c, step k) is stored field by field at rec[tile][field][k][c], so that the threads of the scan
+// kernels (thread = chunk c) read consecutive doubles.  Padding positions (p >= N) get a massless particle.
+// =========================================================================================================
+struct Rec { double r, rinv, ct, st, cp, sp, mass; };
+
+__device__ __forceinline__ Rec load_rec(const double* __restrict__ rec_tile, int k, int c) {
+    const double* b = rec_tile + k * kMexThreads + c;
+    Rec p;
+    p.r = b[0 * kMexTile]; p.rinv = b[1 * kMexTile]; p.ct = b[2 * kMexTile]; p.st = b[3 * kMexTile];
+    p.cp = b[4 * kMexTile]; p.sp = b[5 * kMexTile]; p.mass = b[6 * kMexTile];
+    return p;
+}
+
+__global__ void __launch_bounds__(256)
+mex_gather_kernel(const double* __restrict__ pos, const double* __restrict__ mass, const unsigned* __restrict__ perm,
+                  long long N, long long tiles, double* __restrict__ rec, unsigned* __restrict__ idxT) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= tiles * kMexTile) return;
+    const long long tile = gid / kMexTile;
+    const int rem = (int)(gid - tile * kMexTile);
+    const int k = rem / kMexThreads, c = rem - k * kMexThreads;
+    const long long p = tile * kMexTile + (long long)c * kMexK + k;
+    double x = 1.0, y = 0.0, z = 0.0, mk = 0.0;
+    unsigned i = 0;
+    if (p < N) { i = perm[p]; x = pos[i]; y = pos[N + i]; z = pos[2 * N + i]; mk = mass[i]; }
+    const Geom g = geometry(x, y, z);
+    double* b = rec + (size_t)tile * kRecFields * kMexTile + rem;
+    b[0 * kMexTile] = g.r; b[1 * kMexTile] = g.rinv; b[2 * kMexTile] = g.ct; b[3 * kMexTile] = g.st;
+    b[4 * kMexTile] = g.cp; b[5 * kMexTile] = g.sp; b[6 * kMexTile] = mk;
+    idxT[(size_t)tile * kMexTile + rem] = i;
+}
+
+// =========================================================================================================
+// Per-particle column arithmetic (eqs. 15–17; real form and weights: DESIGN.md "Readings").
+// Column m, stable l-recurrence (never the paper's eq. 24):
+//   m = 0 : P_0 = 1, P_1 = ct, l P_l = (2l-1) ct P_{l-1} - (l-1) P_{l-2}
+//   m >= 1: U_mm = (2m-1)!! st^(m-1), U_{m+1,m} = (2m+1) ct U_mm, (l-m) U_l = (2l-1) ct U_{l-1} - (l+m-1) U_{l-2},
+//           P_lm = st U_lm   (U_lm = P_lm / sin theta is a polynomial: nothing is divided by sin theta)
+// Same-column derivative: dP_lm/dtheta = l ct U_lm - (l+m) U_{l-1,m} (m >= 1);  dP_l0/dtheta = -st U_l1.
+// =========================================================================================================
+template <int LMAX>
+struct Angles {
+    double cm[LMAX + 1], sm[LMAX + 1];   // cos m phi, sin m phi
+    double sp1[LMAX + 1];                // st^(m-1), m >= 1
+    __device__ __forceinline__ void init(const Rec& p) {
+        cm[0] = 1.0; sm[0] = 0.0; sp1[0] = 0.0;
+#pragma unroll
+        for (int m = 1; m <= LMAX; ++m) {
+            cm[m] = fma(cm[m - 1], p.cp, -sm[m - 1] * p.sp);
+            sm[m] = fma(sm[m - 1], p.cp, cm[m - 1] * p.sp);
+            sp1[m] = (m == 1) ? 1.0 : sp1[m - 1] * p.st;
+        }
+    }
+};
+
+// moments of one particle into the running sums of group G (both directions): q[], pq[] have NS entries
+template <int LMAX, int G>
+__device__ __forceinline__ void mex_agg_particle(const Rec& p, double* __restrict__ q, double* __restrict__ pq) {
+    Angles<LMAX> a;
+    a.init(p);
+    double mq[LMAX + 1], mp[LMAX + 1];   // m r^l, m r^-(l+1)
+    mq[0] = p.mass; mp[0] = p.mass * p.rinv;
+#pragma unroll
+    for (int l = 1; l <= LMAX; ++l) { mq[l] = mq[l - 1] * p.r; mp[l] = mp[l - 1] * p.rinv; }
+#pragma unroll
+    for (int m = 0; m <= LMAX; ++m) {
+        if (mex_group_of(LMAX, m) != G) continue;
+        const int sb = mex_slot_base(LMAX, m);
+        double P1 = 0.0, P2 = 0.0;   // P_{l-1,m}, P_{l-2,m}
+#pragma unroll
+        for (int l = m; l <= LMAX; ++l) {
+            double P;
+            if (l == m) P = (m == 0) ? 1.0 : mex_dfact(m) * a.sp1[m] * p.st;
+            else if (l == m + 1) P = double(2 * m + 1) * p.ct * P1;
+            else P = fma(double(2 * l - 1) / double(l - m) * p.ct, P1, -(double(l + m - 1) / double(l - m)) * P2);
+            P2 = P1; P1 = P;
+            const double tq = (mex_w(l, m) * mq[l]) * P, tp = (mex_w(l, m) * mp[l]) * P;
+            if (m == 0) {
+                q[sb + l] += tq;
+                pq[sb + l] += tp;
+            } else {
+                const int s = sb + 2 * (l - m);
+                q[s] = fma(tq, a.cm[m], q[s]);       q[s + 1] = fma(tq, a.sm[m], q[s + 1]);
+                pq[s] = fma(tp, a.cm[m], pq[s]);     pq[s + 1] = fma(tp, a.sm[m], pq[s + 1]);
+            }
+        }
+    }
+}
+
+// Evaluate the group-G part of (Phi, a_r, a_theta, a_phi) at one particle from the running sums s[] of one
+// direction, THEN add the particle's own moment (exclusive sums, eqs. 11–12).
+//   FWD: s = q (interior), radial factor r^-(l+1), d/dr factor -(l+1)/r;  own moment m r^l
+//   BWD: s = p (exterior), radial factor r^l,      d/dr factor  l/r;      own moment m r^-(l+1)
+// out[0..3] += (Phi, a_r, a_theta, a_phi) contributions.
+template <int LMAX, int G, bool FWD>
+__device__ __forceinline__ void mex_eval_particle(const Rec& p, double* __restrict__ s, double* __restrict__ out) {
+    Angles<LMAX> a;
+    a.init(p);
+    double rho[LMAX + 1], mu[LMAX + 1];
+    if (FWD) { rho[0] = p.rinv; mu[0] = p.mass; } else { rho[0] = 1.0; mu[0] = p.mass * p.rinv; }
+#pragma unroll
+    for (int l = 1; l <= LMAX; ++l) {
+        rho[l] = rho[l - 1] * (FWD ? p.rinv : p.r);
+        mu[l] = mu[l - 1] * (FWD ? p.r : p.rinv);
+    }
+    double sP = 0.0, sR = 0.0, sT = 0.0, sF = 0.0;
+#pragma unroll
+    for (int m = 0; m <= LMAX; ++m) {
+        if (mex_group_of(LMAX, m) != G) continue;
+        const int sb = mex_slot_base(LMAX, m);
+        double U1 = 0.0, U2 = 0.0;   // U_{l-1}, U_{l-2} of this column (P for m = 0)
+        double W1 = 0.0, W2 = 0.0;   // m = 0 only: the m = 1 column U_{l-1,1}, U_{l-2,1} for dP_l0/dtheta
+#pragma unroll
+        for (int l = m; l <= LMAX; ++l) {
+            double U;
+            if (l == m) U = (m == 0) ? 1.0 : mex_dfact(m) * a.sp1[m];
+            else if (l == m + 1) U = double(2 * m + 1) * p.ct * U1;
+            else U = fma(double(2 * l - 1) / double(l - m) * p.ct, U1, -(double(l + m - 1) / double(l - m)) * U2);
+            const double kappa = FWD ? -double(l + 1) : double(l);
+            if (m == 0) {
+                double W = 0.0;   // U_{l,1}
+                if (l == 1) W = 1.0;
+                else if (l == 2) W = 3.0 * p.ct;
+                else if (l > 2) W = fma(double(2 * l - 1) / double(l - 1) * p.ct, W1, -(double(l) / double(l - 1)) * W2);
+                W2 = W1; W1 = W;
+                const double e = rho[l] * s[sb + l];
+                const double ye = U * e;
+                sP += ye;
+                sR = fma(kappa, ye, sR);
+                sT = fma(-p.st * W, e, sT);
+                s[sb + l] = fma(mex_w(l, 0) * mu[l], U, s[sb + l]);
+            } else {
+                const int i = sb + 2 * (l - m);
+                const double E = fma(s[i], a.cm[m], s[i + 1] * a.sm[m]);
+                const double F = fma(s[i + 1], a.cm[m], -s[i] * a.sm[m]);
+                const double e = rho[l] * E, f = rho[l] * F;
+                const double Y = p.st * U;
+                const double T = fma(double(l) * p.ct, U, -double(l + m) * U1);
+                const double ye = Y * e;
+                sP += ye;
+                sR = fma(kappa, ye, sR);
+                sT = fma(T, e, sT);
+                sF = fma(double(m) * U, f, sF);
+                const double t = (mex_w(l, m) * mu[l]) * Y;
+                s[i] = fma(t, a.cm[m], s[i]);
+                s[i + 1] = fma(t, a.sm[m], s[i + 1]);
+            }
+            U2 = U1; U1 = U;
+        }
+    }
+    out[0] -= sP;
+    out[1] = fma(p.rinv, sR, out[1]);
+    out[2] = fma(p.rinv, sT, out[2]);
+    out[3] = fma(p.rinv, sF, out[3]);
+}
+
+// =========================================================================================================
+// M4 + M5a: chunk aggregates and the tile-level exclusive scans.
+// Shared memory: V[row][kMexThreads + 1] (row = slot of q, then slot of p), SG[row][4] segment totals.
+// =========================================================================================================
+constexpr int kVStride = kMexThreads + 1;
+constexpr int kSegs = kMexThreads / 32;
+
+template <int LMAX, int G>
+__device__ __forceinline__ void mex_aggregate_group(const double* __restrict__ rec_tile, double* V, double* SG,
+                                                    double* __restrict__ pre, double* __restrict__ tot,
+                                                    long long chunks, long long tiles, long long tile) {
+    constexpr int NS = mex_group_slots(LMAX, G);
+    constexpr int RB = mex_row_base(LMAX, G);
+    constexpr int ROWS = 2 * NS;
+    const int c = threadIdx.x;
+    double q[NS], pq[NS];
+#pragma unroll
+    for (int s = 0; s < NS; ++s) { q[s] = 0.0; pq[s] = 0.0; }
+#pragma unroll 1
+    for (int k = 0; k < kMexK; ++k) {
+        const Rec p = load_rec(rec_tile, k, c);
+        mex_agg_particle<LMAX, G>(p, q, pq);
+    }
+#pragma unroll
+    for (int s = 0; s < NS; ++s) { V[s * kVStride + c] = q[s]; V[(NS + s) * kVStride + c] = pq[s]; }
+    __syncthreads();
+    // segment-local exclusive scans: q rows inside-out (ascending chunk), p rows outside-in (descending chunk)
+    for (int task = c; task < ROWS * kSegs; task += kMexThreads) {
+        const int seg = task / ROWS, row = task - seg * ROWS;
+        const bool fwd = row < NS;
+        double* v = V + row * kVStride + seg * 32;
+        double run = 0.0;
+#pragma unroll 4
+        for (int i = 0; i < 32; ++i) {
+            const int j = fwd ? i : 31 - i;
+            const double t = v[j];
+            v[j] = run;
+            run += t;
+        }
+        SG[row * kSegs + seg] = run;
+    }
+    __syncthreads();
+    const int seg = c >> 5;
+    const long long chunk = tile * kMexThreads + c;
+#pragma unroll 4
+    for (int row = 0; row < ROWS; ++row) {
+        const bool fwd = row < NS;
+        double off = 0.0;
+        if (fwd) { for (int s = 0; s < seg; ++s) off += SG[row * kSegs + s]; }
+        else     { for (int s = kSegs - 1; s > seg; --s) off += SG[row * kSegs + s]; }
+        pre[(size_t)(RB + row) * chunks + chunk] = off + V[row * kVStride + c];
+    }
+    if (c < ROWS) {
+        double t = 0.0;
+        const bool fwd = c < NS;
+        if (fwd) { for (int s = 0; s < kSegs; ++s) t += SG[c * kSegs + s]; }
+        else     { for (int s = kSegs - 1; s >= 0; --s) t += SG[c * kSegs + s]; }
+        tot[(size_t)(RB + c) * tiles + tile] = t;
+    }
+    __syncthreads();
+}
+
+template <int LMAX>
+__global__ void __launch_bounds__(kMexThreads)
+mex_aggregate_kernel(const double* __restrict__ rec, double* __restrict__ pre, double* __restrict__ tot,
+                     long long chunks, long long tiles) {
+    extern __shared__ __align__(16) double smem_d[];
+    constexpr int MAXROWS = 2 * mex_max_group_slots(LMAX);
+    double* V = smem_d;
+    double* SG = smem_d + MAXROWS * kVStride;
+    const long long tile = blockIdx.x;
+    const double* rec_tile = rec + (size_t)tile * kRecFields * kMexTile;
+    constexpr int NG = mex_num_groups(LMAX);
+    mex_aggregate_group<LMAX, 0>(rec_tile, V, SG, pre, tot, chunks, tiles, tile);
+    if constexpr (NG > 1) mex_aggregate_group<LMAX, 1>(rec_tile, V, SG, pre, tot, chunks, tiles, tile);
+    if constexpr (NG > 2) mex_aggregate_group<LMAX, 2>(rec_tile, V, SG, pre, tot, chunks, tiles, tile);
+    if constexpr (NG > 3) mex_aggregate_group<LMAX, 3>(rec_tile, V, SG, pre, tot, chunks, tiles, tile);
+}
+
+// =========================================================================================================
+// M5b: exclusive scan of the tile totals, one block per row, fixed order.  Rows [rb, rb+ns) of a group run
+// forward (q), rows [rb+ns, rb+2ns) backward (p).
+// =========================================================================================================
+struct RowDirs { int ng; int rb[4]; int ns[4]; };
+
+__global__ void __launch_bounds__(256)
+mex_tilescan_kernel(double* __restrict__ tot, long long tiles, RowDirs rd) {
+    __shared__ double sums[256];
+    const int row = blockIdx.x, t = threadIdx.x;
+    bool fwd = true;
+    for (int g = 0; g < rd.ng; ++g)
+        if (row >= rd.rb[g] && row < rd.rb[g] + 2 * rd.ns[g]) fwd = row < rd.rb[g] + rd.ns[g];
+    double* v = tot + (size_t)row * tiles;
+    const long long seg = (tiles + 255) / 256;
+    const long long j0 = (long long)t * seg, j1 = (j0 + seg < tiles) ? j0 + seg : tiles;   // scan-order positions
+    double local = 0.0;
+    for (long long j = j0; j < j1; ++j) local += v[fwd ? j : tiles - 1 - j];
+    sums[t] = local;
+    __syncthreads();
+    double run = 0.0;
+    for (int u = 0; u < t; ++u) run += sums[u];
+    for (long long j = j0; j < j1; ++j) {
+        const long long i = fwd ? j : tiles - 1 - j;
+        const double x = v[i];
+        v[i] = run;
+        run += x;
+    }
+}
+
+// =========================================================================================================
+// M5c + M6 + M7: walk, evaluate, transform, scatter.
+// Shared memory: out[k][4][thread] (Phi, a_r, a_theta, a_phi of the thread's K particles).
+// =========================================================================================================
+template <int LMAX, int G>
+__device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ rec_tile, double* sOut,
+                                                   const double* __restrict__ pre, const double* __restrict__ tot,
+                                                   long long chunks, long long tiles, long long tile) {
+    constexpr int NS = mex_group_slots(LMAX, G);
+    constexpr int RB = mex_row_base(LMAX, G);
+    const int c = threadIdx.x;
+    const long long chunk = tile * kMexThreads + c;
+    double s[NS];
+    // inside-out: q
+#pragma unroll
+    for (int i = 0; i < NS; ++i) s[i] = pre[(size_t)(RB + i) * chunks + chunk] + tot[(size_t)(RB + i) * tiles + tile];
+#pragma unroll 1
+    for (int k = 0; k < kMexK; ++k) {
+        const Rec p = load_rec(rec_tile, k, c);
+        double o[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) o[j] = sOut[(k * 4 + j) * kMexThreads + c];
+        mex_eval_particle<LMAX, G, true>(p, s, o);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) sOut[(k * 4 + j) * kMexThreads + c] = o[j];
+    }
+    // outside-in: p
+#pragma unroll
+    for (int i = 0; i < NS; ++i)
+        s[i] = pre[(size_t)(RB + NS + i) * chunks + chunk] + tot[(size_t)(RB + NS + i) * tiles + tile];
+#pragma unroll 1
+    for (int k = kMexK - 1; k >= 0; --k) {
+        const Rec p = load_rec(rec_tile, k, c);
+        double o[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) o[j] = sOut[(k * 4 + j) * kMexThreads + c];
+        mex_eval_particle<LMAX, G, false>(p, s, o);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) sOut[(k * 4 + j) * kMexThreads + c] = o[j];
+    }
+}
+
+template <int LMAX>
+__global__ void __launch_bounds__(kMexThreads)
+mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__ idxT,
+                    const double* __restrict__ pre, const double* __restrict__ tot,
+                    long long chunks, long long tiles, long long N,
+                    double* __restrict__ acc, double* __restrict__ pot) {
+    __shared__ double sOut[kMexK * 4 * kMexThreads];
+    const long long tile = blockIdx.x;
+    const int c = threadIdx.x;
+    const double* rec_tile = rec + (size_t)tile * kRecFields * kMexTile;
+#pragma unroll
+    for (int i = 0; i < kMexK * 4; ++i) sOut[i * kMexThreads + c] = 0.0;   // thread-private column: no barrier needed
+    constexpr int NG = mex_num_groups(LMAX);
+    mex_evaluate_group<LMAX, 0>(rec_tile, sOut, pre, tot, chunks, tiles, tile);
+    if constexpr (NG > 1) mex_evaluate_group<LMAX, 1>(rec_tile, sOut, pre, tot, chunks, tiles, tile);
+    if constexpr (NG > 2) mex_evaluate_group<LMAX, 2>(rec_tile, sOut, pre, tot, chunks, tiles, tile);
+    if constexpr (NG > 3) mex_evaluate_group<LMAX, 3>(rec_tile, sOut, pre, tot, chunks, tiles, tile);
+#pragma unroll 1
+    for (int k = 0; k < kMexK; ++k) {
+        const long long p = tile * kMexTile + (long long)c * kMexK + k;
+        if (p >= N) continue;
+        const Rec r = load_rec(rec_tile, k, c);
+        const unsigned i = idxT[(size_t)tile * kMexTile + k * kMexThreads + c];
+        Geom g;
+        g.r = r.r; g.rinv = r.rinv; g.ct = r.ct; g.st = r.st; g.cp = r.cp; g.sp = r.sp;
+        double ax, ay, az;
+        to_cartesian(g, sOut[(k * 4 + 1) * kMexThreads + c], sOut[(k * 4 + 2) * kMexThreads + c],
+                     sOut[(k * 4 + 3) * kMexThreads + c], ax, ay, az);
+        acc[i] = ax;
+        acc[N + i] = ay;
+        acc[2 * N + i] = az;
+        pot[i] = sOut[(k * 4 + 0) * kMexThreads + c];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Host side.
+// ---------------------------------------------------------------------------------------------------------
+static cudaError_t mex_sort_enqueue(const double* pos, long long N, const MexLayout& L, char* ws,
+                                    unsigned long long* keys_out, unsigned* idx_out, cudaStream_t st) {
+    unsigned* hist = reinterpret_cast<unsigned*>(ws + L.off_hist);
+    unsigned* tickets = reinterpret_cast<unsigned*>(ws + L.off_ticket);
+    unsigned long long* status = reinterpret_cast<unsigned long long*>(ws + L.off_status);
+    unsigned long long* kbuf[2] = {reinterpret_cast<unsigned long long*>(ws + L.off_keysA),
+                                   reinterpret_cast<unsigned long long*>(ws + L.off_keysB)};
+    unsigned* ibuf[2] = {reinterpret_cast<unsigned*>(ws + L.off_idxA), reinterpret_cast<unsigned*>(ws + L.off_idxB)};
+
+    cudaError_t e = cudaMemsetAsync(ws + L.off_zero, 0, L.zero_bytes, st);
+    if (e != cudaSuccess) return e;
+    long long kg_blocks = (N + 255) / 256;
+    if (kg_blocks > 148 * 8) kg_blocks = 148 * 8;
+    mex_keygen_kernel<<<(unsigned)kg_blocks, 256, 0, st>>>(pos, N, kbuf[0], ibuf[0], hist);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    static bool attr_set = false;
+    if (!attr_set) {
+        e = cudaFuncSetAttribute(mex_radix_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    for (int pass = 0; pass < kSortPasses; ++pass) {
+        const bool last = pass == kSortPasses - 1;
+        mex_radix_pass_kernel<<<(unsigned)L.sort_tiles, kSortThreads, sizeof(SortSmem), st>>>(
+            kbuf[pass & 1], ibuf[pass & 1], last ? keys_out : kbuf[(pass + 1) & 1], last ? idx_out : ibuf[(pass + 1) & 1],
+            N, pass, hist, tickets, status);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+cudaError_t mex_sort_launch(const double* pos, long long N, unsigned long long* keys_sorted, unsigned int* perm,
+                            void* ws, cudaStream_t st) {
+    const MexLayout L = make_mex_layout(N, 0);
+    return mex_sort_enqueue(pos, N, L, static_cast<char*>(ws), keys_sorted, perm, st);
+}
+
+template <int LMAX>
+static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, double* acc, double* pot, cudaStream_t st) {
+    const double* rec = reinterpret_cast<const double*>(ws + L.off_rec);
+    const unsigned* idxT = reinterpret_cast<const unsigned*>(ws + L.off_idxT);
+    double* pre = reinterpret_cast<double*>(ws + L.off_pre);
+    double* tot = reinterpret_cast<double*>(ws + L.off_tot);
+    constexpr int MAXROWS = 2 * mex_max_group_slots(LMAX);
+    const size_t smem = (size_t)(MAXROWS * kVStride + MAXROWS * kSegs) * sizeof(double);
+    auto agg = mex_aggregate_kernel<LMAX>;
+    cudaError_t e = cudaFuncSetAttribute(agg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    agg<<<(unsigned)L.tiles, kMexThreads, smem, st>>>(rec, pre, tot, L.chunks, L.tiles);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    RowDirs rd{};
+    rd.ng = mex_num_groups(LMAX);
+    for (int g = 0; g < rd.ng; ++g) { rd.rb[g] = mex_row_base(LMAX, g); rd.ns[g] = mex_group_slots(LMAX, g); }
+    mex_tilescan_kernel<<<mex_total_rows(LMAX), 256, 0, st>>>(tot, L.tiles, rd);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    mex_evaluate_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(rec, idxT, pre, tot, L.chunks, L.tiles, N, acc, pot);
+    return cudaGetLastError();
+}
+
+cudaError_t mex_force_launch(const double* pos, const double* mass, long long N, int lmax,
+                             double* acc, double* pot, void* wsv, cudaStream_t st) {
+    const MexLayout L = make_mex_layout(N, lmax);
+    char* ws = static_cast<char*>(wsv);
+    unsigned long long* keysA = reinterpret_cast<unsigned long long*>(ws + L.off_keysA);
+    unsigned* idxA = reinterpret_cast<unsigned*>(ws + L.off_idxA);
+    cudaError_t e = mex_sort_enqueue(pos, N, L, ws, keysA, idxA, st);   // pass 7 reads buffer B, writes buffer A
+    if (e != cudaSuccess) return e;
+    const long long gthreads = L.tiles * kMexTile;
+    mex_gather_kernel<<<(unsigned)((gthreads + 255) / 256), 256, 0, st>>>(
+        pos, mass, idxA, N, L.tiles, reinterpret_cast<double*>(ws + L.off_rec), reinterpret_cast<unsigned*>(ws + L.off_idxT));
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    switch (lmax) {
+#define ETICS_CASE(LM) case LM: return mex_scan_enqueue<LM>(L, ws, N, acc, pot, st);
+        ETICS_CASE(0) ETICS_CASE(1) ETICS_CASE(2) ETICS_CASE(3) ETICS_CASE(4) ETICS_CASE(5)
+        ETICS_CASE(6) ETICS_CASE(7) ETICS_CASE(8) ETICS_CASE(9) ETICS_CASE(10)
+#undef ETICS_CASE
+        default: return cudaErrorInvalidValue;
+    }
+}
+
 }  // namespace etics

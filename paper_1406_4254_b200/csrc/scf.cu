@@ -24,7 +24,7 @@ cudaError_t scf_init_constants() { return etics_upload_constants(); }
 // registers; the n loop is a runtime loop.  Loop order l -> n -> m as in PAPER.md:251.
 //
 // Per level l (alpha = 2l+3/2, xi = (r-1)/(r+1), u = 1/(1+r), s = r u^2):
-//   Phi~_nl = f_l C_n(xi),  f_l = -u s^l;   dPhi~_nl/dr = f_l ( g_l C_n + 2 u^2 C'_n ),  g_l = l xi / r - u
+//   Phi~_nl = f_l C_n(xi),  f_l = -u s^l;   dPhi~_nl/dr = f_l ( g_l C_n + 2 u^2 C'_n ),  g_l = f_l'/f_l = -u - l xi / r
 //   SA_m = sum_n A_nlm C_n, SAd_m = sum_n A_nlm C'_n (SB, SBd likewise)  -> 4 FMA per (n,l,m), operand from smem
 //   E_m = SA_m cos(m phi) + SB_m sin(m phi), Ed_m likewise with SAd/SBd, F_m = SB_m cos - SA_m sin
 //   Phi   += f_l sum_m P_lm E_m
@@ -142,7 +142,7 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
         s_t = fma(fl, lv_t, s_t);
         s_f = fma(fl, lv_f, s_f);
         fl *= s;
-        gl += xr;
+        gl -= xr;
 #pragma unroll
         for (int m = 0; m <= l; ++m) { U2[m] = U1[m]; U1[m] = U0[m]; }
     }

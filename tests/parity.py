@@ -16,7 +16,9 @@ def rel_err_scalar(x, ref, floor=FLOOR):
     x = np.asarray(x, dtype=np.float64)
     ref = np.asarray(ref, dtype=np.float64)
     scale = np.maximum(np.abs(ref), floor * np.max(np.abs(ref)))
-    return float(np.max(np.abs(x - ref) / scale))
+    with np.errstate(divide="ignore", invalid="ignore"):
+        e = np.where(scale > 0.0, np.abs(x - ref) / scale, np.where(x == ref, 0.0, np.inf))
+    return float(np.max(e))
 
 
 def rel_err_vector(a, ref):
@@ -25,4 +27,6 @@ def rel_err_vector(a, ref):
     ref = np.asarray(ref, dtype=np.float64)
     num = np.sqrt(np.sum((a - ref) ** 2, axis=0))
     den = np.sqrt(np.sum(ref ** 2, axis=0))
-    return float(np.max(num / den))
+    with np.errstate(divide="ignore", invalid="ignore"):
+        e = np.where(den > 0.0, num / den, np.where(num == 0.0, 0.0, np.inf))   # 0 vs 0 (e.g. innermost particle, lmax=0) agrees
+    return float(np.max(e))
