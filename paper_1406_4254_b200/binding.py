@@ -23,7 +23,7 @@ ETICS_WS_SCF_COEFFS, ETICS_WS_SCF_FORCE, ETICS_WS_MEX_FORCE = 0, 1, 2
 EXPORTS = [
     "etics_status_string", "etics_init", "etics_workspace_bytes", "etics_scf_coeffs", "etics_scf_force",
     "etics_mex_force", "etics_mex_sort", "etics_host_scratch_bytes", "etics_scf_full_host",
-    "etics_mex_full_host", "etics_probe_dfma", "etics_probe_copy",
+    "etics_mex_full_host", "etics_mex_force_timed", "etics_probe_dfma", "etics_probe_copy",
 ]
 
 _lib = None
@@ -66,6 +66,8 @@ def lib() -> C.CDLL:
     L.etics_scf_full_host.argtypes = [_vp, _vp, _ll, _i, _i, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
     L.etics_mex_full_host.restype = _i
     L.etics_mex_full_host.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _vp, _sz, _vp]
+    L.etics_mex_force_timed.restype = _i
+    L.etics_mex_force_timed.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _vp, _sz, _vp, C.POINTER(C.c_float)]
     L.etics_probe_dfma.restype = _i
     L.etics_probe_dfma.argtypes = [_i, _vp, C.POINTER(C.c_double), _vp]
     L.etics_probe_copy.restype = _i
@@ -158,6 +160,19 @@ def etics_mex_force(pos, mass, lmax: int, acc=None, pot=None, workspace=None, st
                               workspace.data_ptr(), wsb, _stream(stream))
     _check(s, "etics_mex_force")
     return acc, pot
+
+
+MEX_STAGES = ("keygen", "radix_passes", "gather", "aggregate", "tilescan", "evaluate")
+
+
+def etics_mex_force_timed(pos, mass, lmax: int, acc, pot, workspace, stream=None):
+    """etics_mex_force with CUDA events between the stages; synchronises; returns {stage: ms}."""
+    N = mass.shape[0]
+    ms = (C.c_float * 6)()
+    s = lib().etics_mex_force_timed(_dev(pos, "pos"), _dev(mass, "mass"), N, lmax, _dev(acc, "acc"), _dev(pot, "pot"),
+                                    workspace.data_ptr(), workspace.numel() * workspace.element_size(), _stream(stream), ms)
+    _check(s, "etics_mex_force_timed")
+    return dict(zip(MEX_STAGES, [float(v) for v in ms]))
 
 
 def etics_mex_sort(pos, keys_sorted=None, perm=None, workspace=None, stream=None):

@@ -161,6 +161,18 @@ etics_status etics_mex_full_host(const double* pos_h, const double* mass_h, long
     return ETICS_OK;
 }
 
+// ---- measurement support ---------------------------------------------------------------------------------
+etics_status etics_mex_force_timed(const double* pos, const double* mass, long long N, int lmax,
+                                   double* acc, double* pot, void* workspace, size_t workspace_bytes, void* stream,
+                                   float* stage_ms) {
+    etics_status s = check_sizes(N, 0, lmax);
+    if (s != ETICS_OK) return s;
+    if (!pos || !mass || !acc || !pot || !workspace || !stage_ms) return ETICS_ERR_ARG;
+    if (misaligned(pos) || misaligned(mass) || misaligned(acc) || misaligned(pot) || misaligned(workspace)) return ETICS_ERR_ALIGN;
+    if (workspace_bytes < etics_workspace_bytes(ETICS_WS_MEX_FORCE, N, 0, lmax)) return ETICS_ERR_WORKSPACE;
+    return from_cuda(mex_force_timed(pos, mass, N, lmax, acc, pot, workspace, static_cast<cudaStream_t>(stream), stage_ms));
+}
+
 // ---- probes ----------------------------------------------------------------------------------------------
 etics_status etics_probe_dfma(int iters, double* sink, double* flops_out, void* stream) {
     if (iters < 1 || !sink) return ETICS_ERR_ARG;

@@ -37,6 +37,13 @@ __host__ __device__ constexpr int num_lm(int lmax) { return (lmax + 1) * (lmax +
 struct BasisConstants {
     double geg_a[kMaxL + 1][kMaxN + 2];
     double geg_b[kMaxL + 1][kMaxN + 2];
+    // monic forms used by the coefficient accumulation (scales are folded into the final normalisation):
+    //   C_n = g_n Q_n,  Q_n = xi Q_{n-1} - beta_n Q_{n-2},  g_n = prod a_i,  beta_n = b_n / (a_n a_{n-1})
+    //   P_lm = h_lm q_l, q_m = st^m, q_l = ct q_{l-1} - gamma_lm q_{l-2},  h_mm = (2m-1)!!, h_lm = h_{l-1,m} (2l-1)/(l-m)
+    double geg_beta[kMaxL + 1][kMaxN + 2];
+    double geg_scale[kMaxL + 1][kMaxN + 1];
+    double leg_gamma[kMaxL + 1][kMaxL + 1];   // [l][m]
+    double leg_scale[kMaxL + 1][kMaxL + 1];   // [l][m]
     double norm_nl[kMaxL + 1][kMaxN + 1];   // A~_nl
     double N_lm[kMaxLM];
     double w_lm[kMaxLM];
@@ -61,6 +68,31 @@ inline void fill_basis_constants(BasisConstants& c) {
         }
         const long double h1 = 2.0L * l + 1.5L, h2 = 2.0L * l + 2.5L;
         g0 = g0 * (4.0L * l + 3.0L) * (4.0L * l + 4.0L) * (4.0L * l + 5.0L) * (4.0L * l + 6.0L) / (256.0L * h1 * h1 * h2 * h2);
+    }
+    for (int l = 0; l <= kMaxL; ++l) {
+        const long double alpha = 2.0L * l + 1.5L;
+        long double g = 1.0L, aprev = 1.0L;
+        c.geg_beta[l][0] = 0.0; c.geg_beta[l][1] = 0.0; c.geg_scale[l][0] = 1.0;
+        for (int n = 1; n <= kMaxN + 1; ++n) {
+            const long double a = 2.0L * (n + alpha - 1.0L) / n, b = (n + 2.0L * alpha - 2.0L) / n;
+            if (n >= 2) c.geg_beta[l][n] = (double)(b / (a * aprev));
+            g *= a;
+            if (n <= kMaxN) c.geg_scale[l][n] = (double)g;
+            aprev = a;
+        }
+    }
+    for (int m = 0; m <= kMaxL; ++m) {
+        long double h = 1.0L, aprev = 1.0L;
+        for (int k = 1; k <= m; ++k) h *= (2.0L * k - 1.0L);
+        for (int l = 0; l <= kMaxL; ++l) { c.leg_gamma[l][m] = 0.0; c.leg_scale[l][m] = 0.0; }
+        c.leg_scale[m][m] = (double)h;
+        for (int l = m + 1; l <= kMaxL; ++l) {
+            const long double a = (2.0L * l - 1.0L) / (l - m), b = (l + m - 1.0L) / (l - m);
+            if (l >= m + 2) c.leg_gamma[l][m] = (double)(b / (a * aprev));
+            h *= a;
+            c.leg_scale[l][m] = (double)h;
+            aprev = a;
+        }
     }
     for (int l = 0; l <= kMaxL; ++l)
         for (int m = 0; m <= l; ++m) {
@@ -140,6 +172,9 @@ cudaError_t mex_sort_launch(const double* pos, long long N, unsigned long long* 
                             void* ws, cudaStream_t st);
 cudaError_t mex_force_launch(const double* pos, const double* mass, long long N, int lmax,
                              double* acc, double* pot, void* ws, cudaStream_t st);
+
+cudaError_t mex_force_timed(const double* pos, const double* mass, long long N, int lmax, double* acc, double* pot,
+                            void* ws, cudaStream_t st, float* stage_ms);
 
 cudaError_t probe_dfma_launch(int iters, double* sink, double* flops_out, cudaStream_t st);
 cudaError_t probe_copy_launch(void* dst, const void* src, size_t bytes, cudaStream_t st);

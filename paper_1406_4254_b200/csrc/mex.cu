@@ -652,7 +652,8 @@ mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__
 // Host side.
 // ---------------------------------------------------------------------------------------------------------
 static cudaError_t mex_sort_enqueue(const double* pos, long long N, const MexLayout& L, char* ws,
-                                    unsigned long long* keys_out, unsigned* idx_out, cudaStream_t st) {
+                                    unsigned long long* keys_out, unsigned* idx_out, cudaStream_t st,
+                                    cudaEvent_t ev_keygen = nullptr) {
     unsigned* hist = reinterpret_cast<unsigned*>(ws + L.off_hist);
     unsigned* tickets = reinterpret_cast<unsigned*>(ws + L.off_ticket);
     unsigned long long* status = reinterpret_cast<unsigned long long*>(ws + L.off_status);
@@ -667,6 +668,7 @@ static cudaError_t mex_sort_enqueue(const double* pos, long long N, const MexLay
     mex_keygen_kernel<<<(unsigned)kg_blocks, 256, 0, st>>>(pos, N, kbuf[0], ibuf[0], hist);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
+    if (ev_keygen) cudaEventRecord(ev_keygen, st);
     static bool attr_set = false;
     if (!attr_set) {
         e = cudaFuncSetAttribute(mex_radix_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
@@ -691,7 +693,8 @@ cudaError_t mex_sort_launch(const double* pos, long long N, unsigned long long* 
 }
 
 template <int LMAX>
-static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, double* acc, double* pot, cudaStream_t st) {
+static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, double* acc, double* pot, cudaStream_t st,
+                                    cudaEvent_t* ev) {
     const double* rec = reinterpret_cast<const double*>(ws + L.off_rec);
     const unsigned* idxT = reinterpret_cast<const unsigned*>(ws + L.off_idxT);
     double* pre = reinterpret_cast<double*>(ws + L.off_pre);
@@ -704,36 +707,63 @@ static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, d
     agg<<<(unsigned)L.tiles, kMexThreads, smem, st>>>(rec, pre, tot, L.chunks, L.tiles);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
+    if (ev) cudaEventRecord(ev[4], st);
     RowDirs rd{};
     rd.ng = mex_num_groups(LMAX);
     for (int g = 0; g < rd.ng; ++g) { rd.rb[g] = mex_row_base(LMAX, g); rd.ns[g] = mex_group_slots(LMAX, g); }
     mex_tilescan_kernel<<<mex_total_rows(LMAX), 256, 0, st>>>(tot, L.tiles, rd);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
+    if (ev) cudaEventRecord(ev[5], st);
     mex_evaluate_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(rec, idxT, pre, tot, L.chunks, L.tiles, N, acc, pot);
-    return cudaGetLastError();
+    e = cudaGetLastError();
+    if (ev) cudaEventRecord(ev[6], st);
+    return e;
 }
 
-cudaError_t mex_force_launch(const double* pos, const double* mass, long long N, int lmax,
-                             double* acc, double* pot, void* wsv, cudaStream_t st) {
+// ev (optional): 7 events recorded at: start, after keygen, after the radix passes, after gather, after aggregate,
+// after tilescan, after evaluate.
+static cudaError_t mex_force_enqueue(const double* pos, const double* mass, long long N, int lmax,
+                                     double* acc, double* pot, void* wsv, cudaStream_t st, cudaEvent_t* ev) {
     const MexLayout L = make_mex_layout(N, lmax);
     char* ws = static_cast<char*>(wsv);
     unsigned long long* keysA = reinterpret_cast<unsigned long long*>(ws + L.off_keysA);
     unsigned* idxA = reinterpret_cast<unsigned*>(ws + L.off_idxA);
-    cudaError_t e = mex_sort_enqueue(pos, N, L, ws, keysA, idxA, st);   // pass 7 reads buffer B, writes buffer A
+    if (ev) cudaEventRecord(ev[0], st);
+    cudaError_t e = mex_sort_enqueue(pos, N, L, ws, keysA, idxA, st, ev ? ev[1] : nullptr);   // pass 7: buffer B -> A
     if (e != cudaSuccess) return e;
+    if (ev) cudaEventRecord(ev[2], st);
     const long long gthreads = L.tiles * kMexTile;
     mex_gather_kernel<<<(unsigned)((gthreads + 255) / 256), 256, 0, st>>>(
         pos, mass, idxA, N, L.tiles, reinterpret_cast<double*>(ws + L.off_rec), reinterpret_cast<unsigned*>(ws + L.off_idxT));
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
+    if (ev) cudaEventRecord(ev[3], st);
     switch (lmax) {
-#define ETICS_CASE(LM) case LM: return mex_scan_enqueue<LM>(L, ws, N, acc, pot, st);
+#define ETICS_CASE(LM) case LM: return mex_scan_enqueue<LM>(L, ws, N, acc, pot, st, ev);
         ETICS_CASE(0) ETICS_CASE(1) ETICS_CASE(2) ETICS_CASE(3) ETICS_CASE(4) ETICS_CASE(5)
         ETICS_CASE(6) ETICS_CASE(7) ETICS_CASE(8) ETICS_CASE(9) ETICS_CASE(10)
 #undef ETICS_CASE
         default: return cudaErrorInvalidValue;
     }
+}
+
+cudaError_t mex_force_launch(const double* pos, const double* mass, long long N, int lmax,
+                             double* acc, double* pot, void* ws, cudaStream_t st) {
+    return mex_force_enqueue(pos, mass, N, lmax, acc, pot, ws, st, nullptr);
+}
+
+// Measurement support: the same launch sequence with CUDA events between the stages; synchronises the stream.
+cudaError_t mex_force_timed(const double* pos, const double* mass, long long N, int lmax, double* acc, double* pot,
+                            void* ws, cudaStream_t st, float* stage_ms) {
+    cudaEvent_t ev[7];
+    for (auto& x : ev) { cudaError_t e = cudaEventCreate(&x); if (e != cudaSuccess) return e; }
+    cudaError_t e = mex_force_enqueue(pos, mass, N, lmax, acc, pot, ws, st, ev);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess)
+        for (int i = 0; i < 6; ++i) cudaEventElapsedTime(&stage_ms[i], ev[i], ev[i + 1]);
+    for (auto& x : ev) cudaEventDestroy(x);
+    return e;
 }
 
 }  // namespace etics
