@@ -42,7 +42,7 @@ struct BasisConstants {
     //   P_lm = h_lm q_l, q_m = st^m, q_l = ct q_{l-1} - gamma_lm q_{l-2},  h_mm = (2m-1)!!, h_lm = h_{l-1,m} (2l-1)/(l-m)
     double geg_beta[kMaxL + 1][kMaxN + 2];
     double geg_scale[kMaxL + 1][kMaxN + 1];
-    double leg_gamma[kMaxL + 1][kMaxL + 1];   // [l][m]
+    double leg_gamma_T[kMaxL + 1][kMaxL + 2];   // [m][l], zero for l < m+2 (and the slack entry l = kMaxL+1)
     double leg_scale[kMaxL + 1][kMaxL + 1];   // [l][m]
     double norm_nl[kMaxL + 1][kMaxN + 1];   // A~_nl
     double N_lm[kMaxLM];
@@ -84,11 +84,12 @@ inline void fill_basis_constants(BasisConstants& c) {
     for (int m = 0; m <= kMaxL; ++m) {
         long double h = 1.0L, aprev = 1.0L;
         for (int k = 1; k <= m; ++k) h *= (2.0L * k - 1.0L);
-        for (int l = 0; l <= kMaxL; ++l) { c.leg_gamma[l][m] = 0.0; c.leg_scale[l][m] = 0.0; }
+        for (int l = 0; l <= kMaxL + 1; ++l) c.leg_gamma_T[m][l] = 0.0;
+        for (int l = 0; l <= kMaxL; ++l) c.leg_scale[l][m] = 0.0;
         c.leg_scale[m][m] = (double)h;
         for (int l = m + 1; l <= kMaxL; ++l) {
             const long double a = (2.0L * l - 1.0L) / (l - m), b = (l + m - 1.0L) / (l - m);
-            if (l >= m + 2) c.leg_gamma[l][m] = (double)(b / (a * aprev));
+            if (l >= m + 2) c.leg_gamma_T[m][l] = (double)(b / (a * aprev));
             h *= a;
             c.leg_scale[l][m] = (double)h;
             aprev = a;
@@ -128,19 +129,21 @@ inline void fill_basis_constants(BasisConstants& c) {
 struct Geom { double r, rinv, ct, st, cp, sp; };
 
 __device__ __forceinline__ Geom geometry(double x, double y, double z) {
+    // reciprocal square roots (MUFU.RSQ64H + Newton, <= 1 ulp) instead of sqrt + divide: 1/r and 1/rho are what
+    // the path needs, r = r^2 (1/r) and rho = rho^2 (1/rho) follow with one multiply each
     Geom g;
     const double rho2 = fma(y, y, x * x);
     const double r2 = fma(z, z, rho2);
-    const double rho = sqrt(rho2);
-    g.r = sqrt(r2);
-    g.rinv = 1.0 / g.r;
+    g.rinv = rsqrt(r2);
+    g.r = r2 * g.rinv;
     g.ct = z * g.rinv;
-    g.st = rho * g.rinv;
-    if (rho > 0.0) {
-        const double ri = 1.0 / rho;
+    if (rho2 > 0.0) {
+        const double ri = rsqrt(rho2);
+        g.st = (rho2 * ri) * g.rinv;
         g.cp = x * ri;
         g.sp = y * ri;
     } else {
+        g.st = 0.0;
         g.cp = 1.0;
         g.sp = 0.0;
     }

@@ -63,7 +63,7 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
         sm[m] = fma(sm[m - 1], g.cp, cm[m - 1] * g.sp);
     }
 
-    const double u = 1.0 / (1.0 + g.r);
+    const double u = __drcp_rn(1.0 + g.r);
     const double xi = (g.r - 1.0) * u;
     const double s = g.r * u * u;
     const double xr = xi * g.rinv;
@@ -162,319 +162,420 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
 //   R_l[k][n] = m_k Phi~_nl(r_k)                                   (n1 = nmax+1 radial features per level)
 //   Y_l[k][f] = P_l0 | P_lm cos m phi | P_lm sin m phi              (2l+1 real angular features per level,
 //               f = 0 -> (m=0), f = 2m-1 -> cos, f = 2m -> sin)
-// Not tensor-core work (north_star); the fp64 FMA pipe is the roof, so the job is to feed it from registers.
-// Each pass handles P particles:
-//   phase 1  thread = particle: geometry, Gegenbauer and Legendre/trig recurrences in registers; features to
-//            shared memory, one row per feature, particles contiguous (sR[row][k], sY[row][k], row stride P+2).
-//   phase 2  thread = unit (n-chunk of NCH, level l, tile of YT consecutive angular features): a register
-//            tile of NCH x YT accumulators; per two particles NCH + YT LDS.128 feed 2*NCH*YT FMAs.  The block's
-//            threads form `streams` copies of the unit list, each taking its own slice of the pass.
-// Accumulators persist over all passes of the block; at the end the streams are combined in ascending order
-// and the block writes one partial table (2T doubles) to the workspace (no atomics: deterministic).
+// Not tensor-core work (north_star); the fp64 FMA pipe is the roof, and the shared-memory pipe (128 B/clk/SM =
+// 16 doubles per 64 FMAs) is the trap: a feature value that travels through shared memory must feed >= 4 FMAs.
+//
+// Mapping: WARP = output tile ("unit": level l, W <= 4 consecutive angular features, a chunk of 11 radial
+// orders), LANE = particle.  Everything but the particle is warp-uniform, so recurrence coefficients are
+// uniform constant-bank operands and every shared-memory access is a fully coalesced, conflict-free row read.
+//   phase 0  (warps 0-3, thread = particle, pass p+2): geometry, cos/sin(m phi) -> G (double-buffered)
+//   phase 1  (all warps, thread = (particle, column class), pass p+1): monic Legendre columns
+//            q_l = ct q_{l-1} - gamma_lm q_{l-2} times cos/sin(m phi) -> Y rows; radial seeds m_k f_l and xi -> F
+//   phase 2  (warp = unit, lane = particle, pass p): monic Gegenbauer chain R_n = xi R_{n-1} - beta_n R_{n-2}
+//            IN REGISTERS (recomputed by every unit of the level: 2 ops per n against 11 W FMAs — cheaper than
+//            sending 11 more rows through shared memory), acc[n][j] += R_n Y_j.
+// One barrier per pass; the three phases of an iteration work on different passes, so warps drift apart and the
+// latency-bound phases 0/1 overlap the FMA-bound phase 2.  Accumulators persist over all passes of the block;
+// at the end the 32 lanes are combined by a fixed butterfly, replicas (small tables) in ascending order, and
+// the block writes one partial table (no atomics: deterministic).  Tables with more than 16 units are split into
+// unit groups (gridDim.y); a group's blocks recompute phases 0/1 for the levels they need.
 // =========================================================================================================
+constexpr int kAccThreads = 512;
+constexpr int kAccWarps = kAccThreads / 32;
+constexpr int kAccP = 128;              // particles per pass
+constexpr int kAccSteps = kAccP / 32;   // phase-2 steps per pass (one particle per lane per step)
+constexpr int kAccNCH = 11;             // radial orders per unit
+constexpr int kAccWMax = 4;             // angular features per unit
+constexpr int kAccMaxGroups = 8;
+constexpr int kAccGRows = 5 + 2 * kMaxL;   // m f_0, xi, s, ct, st, cos(m phi) m=1..lmax, sin(m phi) m=1..lmax
+
+struct AccUnit { short l, f0, w, n0; };
+struct AccGroup {
+    int nunits, rep;           // units of this group; replicas per unit (rep * nunits <= 16 warps)
+    int la, lb;                // levels whose rows the group needs
+    int nrows;                 // feature rows per buffer: Y rows of levels la..lb (row of (l,f) = l^2 + f - la^2),
+                               // then one seed row per level, then xi
+    AccUnit unit[kAccWarps];
+};
+struct AccPlan {
+    int nmax, lmax, n1, L, T;
+    int ngroups;
+    long long passes, passes_per_block;
+    AccGroup group[kAccMaxGroups];
+};
+
+__device__ __forceinline__ double ldc_volatile(const double* p) {
+    double v;
+    asm volatile("ld.const.f64 %0, [%1];" : "=d"(v) : "l"(__cvta_generic_to_constant(p)));
+    return v;
+}
+
+// LV >= 0: level known at compile time and n0 == 0, so that every beta_n is a constant-bank operand with an
+// immediate offset (no registers held for the recurrence coefficients).  LV < 0: generic (later n-chunks).
+template <int W, int LV>
+__device__ __forceinline__ void acc_unit_steps(const double* __restrict__ F, const AccGroup& g, const AccUnit u,
+                                               int rep, int replica, int lane, double (&acc)[kAccNCH][kAccWMax]) {
+    const int l = (LV >= 0) ? LV : u.l;
+    const int n0 = (LV >= 0) ? 0 : u.n0;
+    const double* __restrict__ beta = c_basis.geg_beta[l];
+    const int ny = (g.lb + 1) * (g.lb + 1) - g.la * g.la;   // Y rows of the group
+    const double* yb = F + (size_t)(l * l - g.la * g.la + u.f0) * kAccP + lane;
+    const double* sb = F + (size_t)(ny + l - g.la) * kAccP + lane;
+    const double* xb = F + (size_t)(ny + g.lb - g.la + 1) * kAccP + lane;
+    for (int step = replica; step < kAccSteps; step += rep) {
+        const int o = step * 32;
+        const double xi = xb[o];
+        double y[W];
+#pragma unroll
+        for (int j = 0; j < W; ++j) y[j] = yb[j * kAccP + o];
+        double r1 = sb[o], r2 = 0.0;   // R_n, R_{n-1} (R_0 = seed; beta_1 = 0 so that R_1 = xi R_0)
+        if (LV < 0) {
+            for (int n = 1; n <= n0; ++n) {   // later chunks: run the chain up to their first order
+                const double rn = fma(xi, r1, -beta[n] * r2);
+                r2 = r1; r1 = rn;
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < kAccNCH; ++i) {
+#pragma unroll
+            for (int j = 0; j < W; ++j) acc[i][j] = fma(r1, y[j], acc[i][j]);
+            if (i + 1 < kAccNCH) {
+                // the coefficient is re-read from the constant bank at every use (a volatile load cannot be
+                // hoisted), so that no register is held for it across the unit's 44 accumulators
+                const double rn = (LV >= 0 && i == 0) ? xi * r1 : fma(xi, r1, -ldc_volatile(beta + n0 + i + 1) * r2);
+                r2 = r1; r1 = rn;
+            }
+        }
+    }
+}
+
+template <int W, int LV = 0>
+__device__ __forceinline__ void acc_unit_level(const double* __restrict__ F, const AccGroup& g, const AccUnit u,
+                                               int rep, int replica, int lane, double (&acc)[kAccNCH][kAccWMax]) {
+    if constexpr (LV > kMaxL) {
+        acc_unit_steps<W, -1>(F, g, u, rep, replica, lane, acc);
+    } else {
+        if (u.n0 == 0 && u.l == LV) {
+            if constexpr (W <= 2 * LV + 1) acc_unit_steps<W, LV>(F, g, u, rep, replica, lane, acc);
+        } else {
+            acc_unit_level<W, LV + 1>(F, g, u, rep, replica, lane, acc);
+        }
+    }
+}
+
 // gamma_lm of the monic Legendre recurrence q_l = ct q_{l-1} - gamma_lm q_{l-2} (column m, l >= m+2)
 __host__ __device__ constexpr double leg_gamma_c(int l, int m) {
     return (l >= m + 2) ? double((l + m - 1) * (l - 1 - m)) / double((2 * l - 1) * (2 * l - 3)) : 0.0;
 }
 
-// Angular rows of column M for one particle: q_M = st^M, q_l = ct q_{l-1} - gamma q_{l-2};
-// rows of level l: q_l0 at l^2, (q_lM cos M phi, q_lM sin M phi) at l^2 + 2M - 1, l^2 + 2M.  yk = sY + k.
-template <int LMAX, int M>
-__device__ __forceinline__ void scf_angular_column(double ct, double st, double cp, double sp, double* yk, int stride) {
-    double cm = 1.0, sm = 0.0, q1 = 1.0, q2 = 0.0;
-#pragma unroll
-    for (int i = 1; i <= M; ++i) {
-        const double c2 = fma(cm, cp, -sm * sp);
-        sm = fma(sm, cp, cm * sp);
-        cm = c2;
-        q1 *= st;
-    }
-#pragma unroll
-    for (int l = M; l <= LMAX; ++l) {
-        if (M == 0) {
-            yk[(l * l) * stride] = q1;
-        } else {
-            yk[(l * l + 2 * M - 1) * stride] = q1 * cm;
-            yk[(l * l + 2 * M) * stride] = q1 * sm;
-        }
-        if (l < LMAX) {
-            const double qn = (l == M) ? ct * q1 : fma(ct, q1, -leg_gamma_c(l + 1, M) * q2);
-            q2 = q1; q1 = qn;
-        }
-    }
-}
-
-template <int LMAX, int M>
-__device__ __forceinline__ void scf_angular_dispatch(int row0, int rmask, double ct, double st, double cp, double sp,
-                                                     double* yk, int stride) {
+// Phase 1, one m-column of one particle (compile-time M): monic q_l = ct q_{l-1} - gamma_lm q_{l-2}, q_M = st^M;
+// rows of level l: q_l0 at l^2, (q_lM cos M phi, q_lM sin M phi) at l^2 + 2M - 1, l^2 + 2M.  Fy already points at
+// the particle's element of (virtual) row 0; rows of levels outside [la, lb] are not stored.
+template <int LMAX, int M, bool FULL>
+__device__ __forceinline__ void acc_column(double ct, double st, const double* __restrict__ G, double* __restrict__ Fy,
+                                           int la, int lb) {
     if constexpr (M <= LMAX) {
-        if ((M & rmask) == row0) scf_angular_column<LMAX, M>(ct, st, cp, sp, yk, stride);
-        scf_angular_dispatch<LMAX, M + 1>(row0, rmask, ct, st, cp, sp, yk, stride);
-    }
-}
-
-// Radial rows of level LV for one particle: monic Gegenbauer Q_n scaled by m_k f_l:
-// R_0 = m f_l, R_1 = xi R_0, R_n = xi R_{n-1} - beta_n R_{n-2}.  rk = sR + k.
-template <int LV>
-__device__ __forceinline__ void scf_radial_level(double f0, double xi, double sv, int n1, const double* __restrict__ beta,
-                                                 double* rk, int stride) {
-    double r0 = f0;
+        double cm = 1.0, sm = 0.0, q1 = 1.0, q2 = 0.0;
+        if (M > 0) { cm = G[(4 + M) * kAccP]; sm = G[(4 + kMaxL + M) * kAccP]; }
 #pragma unroll
-    for (int i = 0; i < LV; ++i) r0 *= sv;
-    double* rp = rk + (LV * n1) * stride;
-    double r1 = xi * r0;
-    rp[0] = r0;
-    if (n1 > 1) rp[stride] = r1;
-    int n = 2;
-#pragma unroll 2
-    for (; n + 1 < n1; n += 2) {
-        r0 = fma(xi, r1, -beta[n] * r0);
-        rp[n * stride] = r0;
-        r1 = fma(xi, r0, -beta[n + 1] * r1);
-        rp[(n + 1) * stride] = r1;
-    }
-    if (n < n1) rp[n * stride] = fma(xi, r1, -beta[n] * r0);
-}
-
-template <int LMAX, int LV>
-__device__ __forceinline__ void scf_radial_dispatch(int row0, int rmask, double f0, double xi, double sv, int n1,
-                                                    double* rk, int stride) {
-    if constexpr (LV <= LMAX) {
-        if ((LV & rmask) == row0) scf_radial_level<LV>(f0, xi, sv, n1, c_basis.geg_beta[LV], rk, stride);
-        scf_radial_dispatch<LMAX, LV + 1>(row0, rmask, f0, xi, sv, n1, rk, stride);
+        for (int i = 0; i < M; ++i) q1 *= st;
+#pragma unroll
+        for (int l = M; l <= LMAX; ++l) {
+            if (FULL || (l >= la && l <= lb)) {
+                if (M == 0) Fy[(l * l) * kAccP] = q1;
+                else { Fy[(l * l + 2 * M - 1) * kAccP] = q1 * cm; Fy[(l * l + 2 * M) * kAccP] = q1 * sm; }
+            }
+            if (l < LMAX) {
+                const double qn = (l == M) ? ct * q1 : fma(ct, q1, -leg_gamma_c(l + 1, M) * q2);
+                q2 = q1; q1 = qn;
+            }
+        }
     }
 }
 
-constexpr int kCoeffThreads = 256;
-constexpr int kCoeffNCH = 11;   // radial features per unit
-constexpr int kCoeffYT = 4;     // angular features per unit
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src));
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-struct CoeffPlan {
-    int nmax, lmax, n1, L, T;
-    int nR, nY;      // feature rows: n1*(lmax+1) radial (+slack), (lmax+1)^2 angular (+slack)
-    int P;           // particles per pass
-    int UL;          // units per n-chunk = sum_l ceil((2l+1)/YT)
-    int nchunks, units, streams;
-    int kper;        // particles per stream per pass (even)
-    int stride;      // doubles per feature row
-    int max_blocks;  // workspace is sized for this many block partials
-    long long passes;
-    size_t smem_bytes;
-};
-
-template <int LMAX>
-__global__ void __launch_bounds__(kCoeffThreads, 2)
+// FULL: the table is a single unit group (la = 0, lb = LMAX): no per-row level tests in phase 1.
+template <int LMAX, bool FULL>
+__global__ void __launch_bounds__(kAccThreads, 1)
 scf_accumulate_kernel(const double* __restrict__ pos, const double* __restrict__ mass, long long N,
-                      CoeffPlan pl, long long passes_per_block, double* __restrict__ partial) {
-    constexpr int NCH = kCoeffNCH, YT = kCoeffYT;
+                      const __grid_constant__ AccPlan pl, double* __restrict__ partial) {
     extern __shared__ __align__(16) double smem[];
-    double* sR = smem;
-    double* sY = smem + (size_t)pl.nR * pl.stride;
+    const AccGroup& g = pl.group[blockIdx.y];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double* sG = smem;                                   // [2][kAccGRows][P]  geometry
+    double* sX = sG + 2 * kAccGRows * kAccP;             // [2][4][P]          raw x, y, z, mass (cp.async landing zone)
+    double* sF = sX + 2 * 4 * kAccP;                     // [2][nrows][P]      features
+    const size_t fbuf = (size_t)g.nrows * kAccP;
+    const int la = FULL ? 0 : g.la, lb = FULL ? LMAX : g.lb;
 
-    const int tid = threadIdx.x;
-    const int n1 = pl.n1, stride = pl.stride;
+    // ---- roles -----------------------------------------------------------------------------------------
+    const int my_unit = warp % g.nunits, my_rep = warp / g.nunits;
+    const bool active = my_rep < g.rep;
+    const AccUnit u = g.unit[my_unit];
+    const int pk = tid & (kAccP - 1), pq = tid / kAccP;   // phase 1: particle, column class (0..3)
 
-    // ---- phase-2 role of this thread -------------------------------------------------------------------
-    const int strm = tid / pl.units;
-    const bool active = strm < pl.streams;
-    const int unit = active ? tid - strm * pl.units : 0;
-    const int uc = unit / pl.UL;                  // n-chunk
-    int uv = unit - uc * pl.UL, ul = 0;           // level and feature tile
-    while (uv >= (2 * ul + 1 + YT - 1) / YT) { uv -= (2 * ul + 1 + YT - 1) / YT; ++ul; }
-    const int un0 = uc * NCH, uf0 = uv * YT;
-    // the stream's slice of the pass: pairs [s*(P/2)/streams, (s+1)*(P/2)/streams)
-    const int kbeg = 2 * (((active ? strm : 0) * (pl.P / 2)) / pl.streams);
-    const int kcnt = 2 * ((((active ? strm : 0) + 1) * (pl.P / 2)) / pl.streams) - kbeg;
-    const double* rrow = sR + (size_t)(ul * n1 + un0) * stride + kbeg;
-    const double* yrow = sY + (size_t)(ul * ul + uf0) * stride + kbeg;
-
-    double acc[NCH][YT];
+    double acc[kAccNCH][kAccWMax];
 #pragma unroll
-    for (int i = 0; i < NCH; ++i)
+    for (int i = 0; i < kAccNCH; ++i)
 #pragma unroll
-        for (int j = 0; j < YT; ++j) acc[i][j] = 0.0;
+        for (int j = 0; j < kAccWMax; ++j) acc[i][j] = 0.0;
 
-    const long long pass0 = (long long)blockIdx.x * passes_per_block;
-    const long long pass1 = min(pl.passes, pass0 + passes_per_block);
+    const long long pass0 = (long long)blockIdx.x * pl.passes_per_block;
+    const long long pass1 = min(pl.passes, pass0 + pl.passes_per_block);
 
-    double* sG = sY + (size_t)pl.nY * stride;   // geometry, double-buffered: 2 x 8 fields x P
-    const int P = pl.P;                          // 32, 64 or 128: tasks (row, k) need no division
-    const int task_k = tid & (P - 1);
-    const int task_row0 = tid / P, task_rmask = kCoeffThreads / P - 1;   // rows row0, row0 + 256/P, ...
-
-    // geometry of particle k of a pass (thread = particle), into buffer `buf`
-    auto phase0 = [&](long long pass, int buf) {
-        if (tid < P && pass < pass1) {
-            double* G = sG + buf * 8 * P;
-            const long long k = pass * P + tid;
-            double x = 1.0, y = 0.0, z = 0.0, mk = 0.0;   // padding particles carry zero mass
-            if (k < N) { x = pos[k]; y = pos[N + k]; z = pos[2 * N + k]; mk = mass[k]; }
-            const Geom g = geometry(x, y, z);
-            const double u = 1.0 / (1.0 + g.r);
-            G[0 * P + tid] = -u * mk;              // m_k f_0,  f_l = -u s^l
-            G[1 * P + tid] = (g.r - 1.0) * u;      // xi
-            G[2 * P + tid] = g.r * u * u;          // s
-            G[3 * P + tid] = g.ct;
-            G[4 * P + tid] = g.st;
-            G[5 * P + tid] = g.cp;
-            G[6 * P + tid] = g.sp;
+    // raw coordinates of a pass: global -> shared with cp.async, thread k moves (and later reads) element k only
+    auto prefetch = [&](long long pass) {
+        if (tid < kAccP && pass < pass1) {
+            const long long k = pass * kAccP + tid;
+            if (k < N) {
+                double* X = sX + (size_t)(pass & 1) * 4 * kAccP + tid;
+                cp_async8(X, pos + k);
+                cp_async8(X + kAccP, pos + N + k);
+                cp_async8(X + 2 * kAccP, pos + 2 * N + k);
+                cp_async8(X + 3 * kAccP, mass + k);
+            }
         }
     };
-    phase0(pass0, 0);
+    auto phase0 = [&](long long pass) {
+        if (tid < kAccP && pass < pass1) {
+            cp_async_wait_all();
+            double* G = sG + (size_t)(pass & 1) * kAccGRows * kAccP + tid;
+            const double* X = sX + (size_t)(pass & 1) * 4 * kAccP + tid;
+            const long long k = pass * kAccP + tid;
+            double x = 1.0, y = 0.0, z = 0.0, mk = 0.0;   // padding particles carry zero mass
+            if (k < N) { x = X[0]; y = X[kAccP]; z = X[2 * kAccP]; mk = X[3 * kAccP]; }
+            const Geom gm = geometry(x, y, z);
+            const double uu = __drcp_rn(1.0 + gm.r);
+            G[0 * kAccP] = -uu * mk;               // m_k f_0,  f_l = -u s^l
+            G[1 * kAccP] = (gm.r - 1.0) * uu;      // xi
+            G[2 * kAccP] = gm.r * uu * uu;         // s
+            G[3 * kAccP] = gm.ct;
+            G[4 * kAccP] = gm.st;
+            double cm = gm.cp, sm = gm.sp;
+#pragma unroll
+            for (int m = 1; m <= LMAX; ++m) {
+                G[(4 + m) * kAccP] = cm;
+                G[(4 + kMaxL + m) * kAccP] = sm;
+                const double c2 = fma(cm, gm.cp, -sm * gm.sp);
+                sm = fma(sm, gm.cp, cm * gm.sp);
+                cm = c2;
+            }
+        }
+    };
+    auto phase1 = [&](long long pass) {
+        if (pass >= pass1) return;
+        const double* G = sG + (size_t)(pass & 1) * kAccGRows * kAccP + pk;
+        double* F = sF + (size_t)(pass & 1) * fbuf + pk;
+        double* Fy = F - (size_t)(la * la) * kAccP;   // row (l, f) of the group's buffer = l^2 + f - la^2
+        const double ct = G[3 * kAccP], st = G[4 * kAccP];
+        switch (pq) {   // warp-uniform: 4 warps per class
+            case 0:
+                acc_column<LMAX, 0, FULL>(ct, st, G, Fy, la, lb); acc_column<LMAX, 7, FULL>(ct, st, G, Fy, la, lb);
+                acc_column<LMAX, 8, FULL>(ct, st, G, Fy, la, lb);
+                break;
+            case 1:
+                acc_column<LMAX, 1, FULL>(ct, st, G, Fy, la, lb); acc_column<LMAX, 6, FULL>(ct, st, G, Fy, la, lb);
+                acc_column<LMAX, 9, FULL>(ct, st, G, Fy, la, lb);
+                break;
+            case 2:
+                acc_column<LMAX, 2, FULL>(ct, st, G, Fy, la, lb); acc_column<LMAX, 5, FULL>(ct, st, G, Fy, la, lb);
+                acc_column<LMAX, 10, FULL>(ct, st, G, Fy, la, lb);
+                break;
+            default: {
+                acc_column<LMAX, 3, FULL>(ct, st, G, Fy, la, lb); acc_column<LMAX, 4, FULL>(ct, st, G, Fy, la, lb);
+                // radial seeds m_k f_l (rows after the Y rows) and xi
+                const double sv = G[2 * kAccP];
+                double f = G[0];
+                double* Fs = F + (size_t)((lb + 1) * (lb + 1) - la * la - la) * kAccP;   // seed row of level l: Fs[l P]
+#pragma unroll
+                for (int l = 0; l <= LMAX; ++l) {
+                    if (FULL || (l >= la && l <= lb)) Fs[l * kAccP] = f;
+                    f *= sv;
+                }
+                Fs[(lb + 1) * kAccP] = G[1 * kAccP];
+            }
+        }
+    };
+
+    // ---- prologue: raw data of passes 0..2, geometry of passes 0 and 1, features of pass 0 ------------------
+    prefetch(pass0);
+    phase0(pass0);
+    prefetch(pass0 + 1);
+    phase0(pass0 + 1);
+    prefetch(pass0 + 2);
+    __syncthreads();
+    phase1(pass0);
     __syncthreads();
 
     for (long long pass = pass0; pass < pass1; ++pass) {
-        const int buf = (int)((pass - pass0) & 1);
-        // ---- phase 1: feature rows of this pass; task = (row, particle k), the row is warp-uniform ------------
-        {
-            const double* G = sG + buf * 8 * P;
-            scf_radial_dispatch<LMAX, 0>(task_row0, task_rmask, G[0 * P + task_k], G[1 * P + task_k], G[2 * P + task_k],
-                                         n1, sR + task_k, stride);
-            scf_angular_dispatch<LMAX, 0>(task_row0, task_rmask, G[3 * P + task_k], G[4 * P + task_k], G[5 * P + task_k],
-                                          G[6 * P + task_k], sY + task_k, stride);
-        }
-        __syncthreads();
-        // ---- phase 0 of the next pass (overlaps phase 2 of the other warps) ---------------------------------
-        phase0(pass + 1, buf ^ 1);
-
-        // ---- phase 2: register-tiled accumulation, two particles per shared-memory load -------------------
-        if (active) {
-#pragma unroll 1
-            for (int k = 0; k < kcnt; k += 2) {
-                double2 yv[YT];
-#pragma unroll
-                for (int j = 0; j < YT; ++j) yv[j] = *reinterpret_cast<const double2*>(yrow + (size_t)j * stride + k);
-#pragma unroll
-                for (int i = 0; i < NCH; ++i) {
-                    const double2 r = *reinterpret_cast<const double2*>(rrow + (size_t)i * stride + k);
-#pragma unroll
-                    for (int j = 0; j < YT; ++j) {
-                        acc[i][j] = fma(r.x, yv[j].x, acc[i][j]);
-                        acc[i][j] = fma(r.y, yv[j].y, acc[i][j]);
-                    }
-                }
+        phase0(pass + 2);     // writes G[pass&1] (last read by phase1(pass), before the previous barrier)
+        prefetch(pass + 3);   // overwrites X[(pass+1)&1], consumed by this thread's phase0(pass+1) one iteration ago
+        phase1(pass + 1);     // reads G[(pass+1)&1] (written before the previous barrier), writes F[(pass+1)&1]
+        if (active) {         // reads F[pass&1] (written before the previous barrier)
+            const double* F = sF + (size_t)(pass & 1) * fbuf;
+            switch (u.w) {
+                case 1: acc_unit_level<1>(F, g, u, g.rep, my_rep, lane, acc); break;
+                case 2: acc_unit_level<2>(F, g, u, g.rep, my_rep, lane, acc); break;
+                case 3: acc_unit_level<3>(F, g, u, g.rep, my_rep, lane, acc); break;
+                default: acc_unit_level<4>(F, g, u, g.rep, my_rep, lane, acc); break;
             }
         }
         __syncthreads();
     }
 
-    // ---- combine the streams in ascending order; one partial table per block ----------------------------
-    double* sOut = smem;   // [2T]: cos table then sin table
-    for (int t = tid; t < 2 * pl.T; t += kCoeffThreads) sOut[t] = 0.0;
+    // ---- lanes -> one value per accumulator (fixed butterfly), replicas in ascending order -----------------
+#pragma unroll
+    for (int i = 0; i < kAccNCH; ++i)
+#pragma unroll
+        for (int j = 0; j < kAccWMax; ++j) {
+            double v = acc[i][j];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            acc[i][j] = v;
+        }
+    double* sOut = smem;   // [2T]: cos table then sin table (entries of other groups stay untouched)
     __syncthreads();
-    for (int sI = 0; sI < pl.streams; ++sI) {
-        if (active && strm == sI) {
+    for (int r = 0; r < g.rep; ++r) {
+        if (active && my_rep == r && lane == 0) {
 #pragma unroll
-            for (int i = 0; i < NCH; ++i)
+            for (int i = 0; i < kAccNCH; ++i)
 #pragma unroll
-                for (int j = 0; j < YT; ++j) {
-                    const int n = un0 + i, f = uf0 + j;
-                    if (n < n1 && f <= 2 * ul) {
+                for (int j = 0; j < kAccWMax; ++j) {
+                    const int n = u.n0 + i, f = u.f0 + j;
+                    if (n < pl.n1 && j < u.w) {
                         const int m = (f + 1) >> 1;
                         const bool is_sin = (f > 0) && ((f & 1) == 0);
-                        sOut[(is_sin ? pl.T : 0) + n * pl.L + lm_index(ul, m)] += acc[i][j];
+                        const int t = (is_sin ? pl.T : 0) + n * pl.L + lm_index(u.l, m);
+                        sOut[t] = (r == 0) ? acc[i][j] : sOut[t] + acc[i][j];
                     }
                 }
         }
         __syncthreads();
     }
-    for (int t = tid; t < 2 * pl.T; t += kCoeffThreads) partial[(size_t)blockIdx.x * 2 * pl.T + t] = sOut[t];
+    if (active && my_rep == 0 && lane == 0) {
+        double* out = partial + (size_t)blockIdx.x * 2 * pl.T;
+#pragma unroll
+        for (int i = 0; i < kAccNCH; ++i)
+#pragma unroll
+            for (int j = 0; j < kAccWMax; ++j) {
+                const int n = u.n0 + i, f = u.f0 + j;
+                if (n < pl.n1 && j < u.w) {
+                    const int m = (f + 1) >> 1;
+                    const bool is_sin = (f > 0) && ((f & 1) == 0);
+                    const int t = (is_sin ? pl.T : 0) + n * pl.L + lm_index(u.l, m);
+                    out[t] = sOut[t];
+                }
+            }
+    }
 }
 
-// S5: fixed-order reduction over block partials and normalisation.
-// Block = 32 outputs (threadIdx.x, coalesced along the table) x kFinSlices slices of the block partials
-// (threadIdx.y); every slice sums its partials b = y, y + kFinSlices, ... in ascending order with four
-// interleaved accumulators, then the slices are combined in ascending y.  The order depends only on `blocks`.
-constexpr int kFinSlices = 16;
+// S5: fixed-order reduction over block partials and normalisation.  One warp per output: lane j sums the
+// partials of blocks j, j+32, ... in ascending order, then a fixed butterfly combines the lanes.  The order
+// depends only on `blocks` (a function of N and the table size), never on scheduling.
+constexpr int kFinThreads = 256;
 
-__global__ void __launch_bounds__(32 * kFinSlices)
+__global__ void __launch_bounds__(kFinThreads)
 scf_finalize_kernel(const double* __restrict__ partial, int blocks, int nmax, int lmax,
                     double* __restrict__ A, double* __restrict__ B) {
-    __shared__ double sh[kFinSlices][33];
     const int L = num_lm(lmax), T = (nmax + 1) * L;
-    const int t = blockIdx.x * 32 + threadIdx.x, y = threadIdx.y;
-    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-    if (t < 2 * T) {
-        int b = y;
-        for (; b + 3 * kFinSlices < blocks; b += 4 * kFinSlices) {
-            s0 += partial[(size_t)(b + 0 * kFinSlices) * 2 * T + t];
-            s1 += partial[(size_t)(b + 1 * kFinSlices) * 2 * T + t];
-            s2 += partial[(size_t)(b + 2 * kFinSlices) * 2 * T + t];
-            s3 += partial[(size_t)(b + 3 * kFinSlices) * 2 * T + t];
-        }
-        for (; b < blocks; b += kFinSlices) s0 += partial[(size_t)b * 2 * T + t];
-    }
-    sh[y][threadIdx.x] = (s0 + s1) + (s2 + s3);
-    __syncthreads();
-    if (y != 0 || t >= 2 * T) return;
-    double sum = 0.0;
-#pragma unroll
-    for (int i = 0; i < kFinSlices; ++i) sum += sh[i][threadIdx.x];
+    const int t = blockIdx.x * (kFinThreads / 32) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (t >= 2 * T) return;
     const int tt = (t < T) ? t : t - T;
     const int n = tt / L, j = tt - n * L;
     int l = 0;
     while (lm_index(l + 1, 0) <= j) ++l;
     const int m = j - lm_index(l, 0);
+    if (t >= T && m == 0) {   // B_{nl0}: no such feature was accumulated
+        if (lane == 0) B[tt] = 0.0;
+        return;
+    }
+    double s = 0.0;
+    for (int b = lane; b < blocks; b += 32) s += partial[(size_t)b * 2 * T + t];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane != 0) return;
     const double norm = (c_basis.norm_nl[l][n] * c_basis.geg_scale[l][n]) * (c_basis.N_lm[j] * c_basis.leg_scale[l][m]);
-    if (t < T) A[tt] = norm * sum;
-    else B[tt] = (m == 0) ? 0.0 : norm * sum;
+    if (t < T) A[tt] = norm * s;
+    else B[tt] = norm * s;
 }
 
 // ---------------------------------------------------------------------------------------------------------
 // Host side: plan, workspace, launches.
 // ---------------------------------------------------------------------------------------------------------
-constexpr int kCoeffMaxBlocks = 148 * 8;
-constexpr size_t kSmemBudget = 227 * 1024;
+constexpr int kAccMaxBlocksX = 148;
 
-static CoeffPlan make_coeff_plan(long long N, int nmax, int lmax) {
-    CoeffPlan p{};
+// Units in (level, n-chunk, feature tile) order; widths as equal as possible (2l+1 features in ceil(./4) tiles).
+static AccPlan make_acc_plan(long long N, int nmax, int lmax) {
+    AccPlan p{};
     p.nmax = nmax; p.lmax = lmax; p.n1 = nmax + 1; p.L = num_lm(lmax); p.T = p.n1 * p.L;
-    p.nchunks = (p.n1 + kCoeffNCH - 1) / kCoeffNCH;
-    p.UL = 0;
-    for (int l = 0; l <= lmax; ++l) p.UL += (2 * l + 1 + kCoeffYT - 1) / kCoeffYT;
-    p.units = p.UL * p.nchunks;
-    // slack rows: the last n-chunk / feature tile of a level reads (and ignores) rows past its level
-    p.nR = p.n1 * (lmax + 1) + (p.nchunks * kCoeffNCH - p.n1);
-    p.nY = (lmax + 1) * (lmax + 1) + (kCoeffYT - 1);
-    auto smem_for = [&](int P) { return ((size_t)(p.nR + p.nY) * (P + 2) + (size_t)16 * P) * sizeof(double); };
-    // P in {128, 64, 32}: the largest that leaves two resident blocks per SM (registers allow two), else the
-    // largest that fits at all
-    int P = 128;
-    while (P > 32 && smem_for(P) > kSmemBudget / 2) P /= 2;
-    if (smem_for(P) > kSmemBudget / 2) { P = 128; while (P > 32 && smem_for(P) > kSmemBudget) P /= 2; }
-    int streams = kCoeffThreads / p.units;
-    if (streams < 1) streams = 1;
-    if (streams > P / 2) streams = P / 2;
-    p.P = P; p.streams = streams; p.kper = 0;
-    p.stride = P + 2;
-    p.smem_bytes = smem_for(P);
-    p.passes = (N + P - 1) / P;
-    p.max_blocks = (int)(p.passes < kCoeffMaxBlocks ? p.passes : kCoeffMaxBlocks);
+    const int nchunks = (p.n1 + kAccNCH - 1) / kAccNCH;
+    AccUnit all[kAccMaxGroups * kAccWarps];
+    int nu = 0;
+    for (int l = 0; l <= lmax; ++l) {
+        const int F = 2 * l + 1, tiles = (F + kAccWMax - 1) / kAccWMax;
+        for (int c = 0; c < nchunks; ++c) {
+            int f0 = 0;
+            for (int t = 0; t < tiles; ++t) {
+                const int w = F / tiles + (t < F % tiles ? 1 : 0);
+                all[nu++] = AccUnit{(short)l, (short)f0, (short)w, (short)(c * kAccNCH)};
+                f0 += w;
+            }
+        }
+    }
+    p.ngroups = (nu + kAccWarps - 1) / kAccWarps;
+    for (int gi = 0; gi < p.ngroups; ++gi) {
+        AccGroup& g = p.group[gi];
+        // groups of (almost) equal size
+        const int u0 = (int)((long long)nu * gi / p.ngroups), u1 = (int)((long long)nu * (gi + 1) / p.ngroups);
+        g.nunits = u1 - u0;
+        g.rep = kAccWarps / g.nunits;
+        if (g.rep > kAccSteps) g.rep = kAccSteps;
+        if (g.rep == 3) g.rep = 2;   // replicas take steps r, r+rep, ... of the 4 steps of a pass
+        g.la = all[u0].l; g.lb = all[u1 - 1].l;
+        // heavier units first is not needed: warp w sits on scheduler w % 4, and consecutive units have
+        // similar widths, so every scheduler gets a similar sum of (W+2) * 11 operations
+        for (int i = 0; i < g.nunits; ++i) g.unit[i] = all[u0 + i];
+        g.nrows = (g.lb + 1) * (g.lb + 1) - g.la * g.la + (g.lb - g.la + 1) + 1;
+    }
+    p.passes = (N + kAccP - 1) / kAccP;
+    long long bx = p.passes < kAccMaxBlocksX ? p.passes : kAccMaxBlocksX;
+    p.passes_per_block = (p.passes + bx - 1) / bx;
     return p;
 }
 
+static int acc_blocks_x(const AccPlan& p) { return (int)((p.passes + p.passes_per_block - 1) / p.passes_per_block); }
+
+static size_t acc_smem_bytes(const AccPlan& p) {
+    int nrows = 0;
+    for (int gi = 0; gi < p.ngroups; ++gi) nrows = p.group[gi].nrows > nrows ? p.group[gi].nrows : nrows;
+    size_t b = (size_t)(2 * kAccGRows + 2 * 4 + 2 * nrows) * kAccP * sizeof(double);
+    const size_t out = (size_t)2 * p.T * sizeof(double);
+    return b > out ? b : out;
+}
+
 size_t scf_coeffs_workspace(long long N, int nmax, int lmax) {
-    CoeffPlan p = make_coeff_plan(N, nmax, lmax);
-    return round_up((size_t)p.max_blocks * 2 * p.T * sizeof(double), 256);
+    (void)N;
+    return round_up((size_t)kAccMaxBlocksX * 2 * (nmax + 1) * num_lm(lmax) * sizeof(double), 256);
 }
 
 template <int LMAX>
-static cudaError_t launch_accumulate(const double* pos, const double* mass, long long N, const CoeffPlan& p,
-                                     double* partial, int* blocks_out, cudaStream_t st) {
-    auto kern = scf_accumulate_kernel<LMAX>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_bytes);
-    if (e != cudaSuccess) return e;
-    // one wave of resident blocks: grid = SMs x blocks per SM (capped by the workspace and by the work)
-    int dev = 0, sms = 0, occ = 0;
-    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
-    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kCoeffThreads, p.smem_bytes)) != cudaSuccess) return e;
-    long long blocks = (long long)sms * (occ > 0 ? occ : 1);
-    if (blocks > p.max_blocks) blocks = p.max_blocks;
-    const long long ppb = (p.passes + blocks - 1) / blocks;
-    blocks = (p.passes + ppb - 1) / ppb;
-    *blocks_out = (int)blocks;
-    kern<<<(unsigned)blocks, kCoeffThreads, p.smem_bytes, st>>>(pos, mass, N, p, ppb, partial);
+static cudaError_t launch_accumulate(const double* pos, const double* mass, long long N, const AccPlan& p, int bx,
+                                     double* partial, cudaStream_t st) {
+    const size_t smem = acc_smem_bytes(p);
+    static size_t smem_set[2] = {0, 0};   // per template instance
+    const bool full = p.ngroups == 1;
+    if (smem > smem_set[full]) {
+        cudaError_t e = full ? cudaFuncSetAttribute(scf_accumulate_kernel<LMAX, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                             : cudaFuncSetAttribute(scf_accumulate_kernel<LMAX, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        smem_set[full] = smem;
+    }
+    if (full) scf_accumulate_kernel<LMAX, true><<<dim3(bx, 1), kAccThreads, smem, st>>>(pos, mass, N, p, partial);
+    else scf_accumulate_kernel<LMAX, false><<<dim3(bx, p.ngroups), kAccThreads, smem, st>>>(pos, mass, N, p, partial);
     return cudaGetLastError();
 }
 
@@ -482,19 +583,19 @@ cudaError_t scf_coeffs_launch(const double* pos, const double* mass, long long N
                               double* A, double* B, void* ws, cudaStream_t st) {
     cudaError_t e = etics_upload_constants();
     if (e != cudaSuccess) return e;
-    const CoeffPlan p = make_coeff_plan(N, nmax, lmax);
+    const AccPlan p = make_acc_plan(N, nmax, lmax);
     double* partial = static_cast<double*>(ws);
-    int blocks = 0;
+    const int bx = acc_blocks_x(p);
     switch (lmax) {
-#define ETICS_CASE(LM) case LM: e = launch_accumulate<LM>(pos, mass, N, p, partial, &blocks, st); break;
+#define ETICS_CASE(LM) case LM: e = launch_accumulate<LM>(pos, mass, N, p, bx, partial, st); break;
         ETICS_CASE(0) ETICS_CASE(1) ETICS_CASE(2) ETICS_CASE(3) ETICS_CASE(4) ETICS_CASE(5)
         ETICS_CASE(6) ETICS_CASE(7) ETICS_CASE(8) ETICS_CASE(9) ETICS_CASE(10)
 #undef ETICS_CASE
         default: return cudaErrorInvalidValue;
     }
     if (e != cudaSuccess) return e;
-    const int T2 = 2 * p.T;
-    scf_finalize_kernel<<<(T2 + 31) / 32, dim3(32, kFinSlices), 0, st>>>(partial, blocks, nmax, lmax, A, B);
+    const int T2 = 2 * p.T, wpb = kFinThreads / 32;
+    scf_finalize_kernel<<<(T2 + wpb - 1) / wpb, kFinThreads, 0, st>>>(partial, bx, nmax, lmax, A, B);
     return cudaGetLastError();
 }
 
