@@ -94,12 +94,15 @@ constexpr int kMexK = 8;
 constexpr int kMexTile = kMexThreads * kMexK;
 constexpr int kRecFields = 8;   // r, 1/r, cos th, sin th, cos ph, sin ph, mass, (spare)
 
-// Radix sort geometry.
+// Radix sort geometry: 256 threads (thread d owns digit d in the offset phase), ITEMS keys per thread.
+// ITEMS = 8 (2048-key tiles): more tiles and a shorter ranking chain per tile — the passes of a small sort are
+// latency bound; ITEMS = 16 (4096-key tiles): longer runs of equal digits per tile for the large sorts.
 constexpr int kSortThreads = 256;
-constexpr int kSortItems = 16;
-constexpr int kSortTile = kSortThreads * kSortItems;
 constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kSortPasses = 8;
+constexpr int kSortMinTile = kSortThreads * 8;     // the status buffer is sized for the smallest tile
+constexpr int kLookW = 16;                         // tiles inspected per look-back round
+constexpr long long kSortSmallN = 1ll << 22;       // N below this: ITEMS = 8
 
 struct MexLayout {
     long long N;
@@ -116,7 +119,7 @@ struct MexLayout {
 static MexLayout make_mex_layout(long long N, int lmax) {
     MexLayout L{};
     L.N = N; L.lmax = lmax;
-    L.sort_tiles = (N + kSortTile - 1) / kSortTile;
+    L.sort_tiles = (N + kSortMinTile - 1) / kSortMinTile;
     L.tiles = (N + kMexTile - 1) / kMexTile;
     L.chunks = L.tiles * kMexThreads;
     L.rows = mex_total_rows(lmax);
@@ -174,20 +177,43 @@ mex_keygen_kernel(const double* __restrict__ pos, long long N, unsigned long lon
 // M2: one stable LSD radix pass (8 bits) with decoupled lookback.
 // status word: [63:56] tag (2*pass+1 = tile aggregate, 2*pass+2 = inclusive prefix, anything else = not yet),
 //              [55:0] count.  The buffer is zeroed once per sort; tags of earlier passes read as "not yet".
+// Ranking: the lanes of a warp that hold the same digit are found with eight ballots (one per digit bit) —
+// the MATCH.ANY instruction iterates over the distinct values of the warp and was the kernel's bottleneck
+// (profiles/r1b_summary.md).  Launched with programmatic stream serialisation: the prologue (ticket, clearing the
+// counters) overlaps the tail of the preceding pass; griddepcontrol.wait orders every read of its output.
 // =========================================================================================================
 constexpr unsigned long long kCountMask = (1ull << 56) - 1;
 
+// Phase timestamps of the radix pass for the development harness (compiled out of the library).
+#ifdef ETICS_SORT_TRACE
+__device__ unsigned long long g_sort_trace[1 << 16][8];
+#define ETICS_TRACE(slot)                                                                              \
+    do {                                                                                               \
+        if (threadIdx.x == 0) {                                                                        \
+            unsigned long long t_;                                                                     \
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                                     \
+            g_sort_trace[blockIdx.x & 0xffff][slot] = t_;                                              \
+        }                                                                                              \
+    } while (0)
+#else
+#define ETICS_TRACE(slot) do {} while (0)
+#endif
+
+template <int ITEMS>
 struct SortSmem {
-    unsigned warp_hist[kSortWarps][256];   // per-warp digit counts -> exclusive offsets of the warp inside the tile
-    unsigned local_off[256];               // exclusive digit offsets inside the tile
+    uint2 warp_hist[kSortWarps][256];      // per warp and digit: .x = match mask of the item being ranked, .y = digit
+                                           // count so far -> exclusive offset of the warp's keys inside the tile
     unsigned gbase[256];                   // global position of the tile's first key of digit d, minus local_off[d]
     unsigned scan_tmp[kSortWarps];
     unsigned tile;
-    unsigned long long keys[kSortTile];
-    unsigned idx[kSortTile];
+    unsigned long long keys[kSortThreads * ITEMS];
+    unsigned idx[kSortThreads * ITEMS];
 };
 
-__device__ __forceinline__ unsigned block_exclusive_scan_256(unsigned v, unsigned* tmp, unsigned* total) {
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+__device__ __forceinline__ unsigned block_exclusive_scan_256(unsigned v, unsigned* tmp) {
     // kSortThreads == 256 threads, one value each
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     unsigned inc = v;
@@ -198,67 +224,80 @@ __device__ __forceinline__ unsigned block_exclusive_scan_256(unsigned v, unsigne
     }
     if (lane == 31) tmp[warp] = inc;
     __syncthreads();
-    unsigned woff = 0, tot = 0;
+    unsigned woff = 0;
 #pragma unroll
     for (int w = 0; w < kSortWarps; ++w) {
         const unsigned t = tmp[w];
         if (w < warp) woff += t;
-        tot += t;
     }
     __syncthreads();
-    if (total) *total = tot;
     return woff + inc - v;
 }
 
-__global__ void __launch_bounds__(kSortThreads)
+template <int ITEMS>
+__global__ void __launch_bounds__(kSortThreads, ITEMS <= 8 ? 4 : 3)
 mex_radix_pass_kernel(const unsigned long long* __restrict__ keys_in, const unsigned* __restrict__ idx_in,
                       unsigned long long* __restrict__ keys_out, unsigned* __restrict__ idx_out,
                       long long N, int pass, const unsigned* __restrict__ hist, unsigned* __restrict__ tickets,
                       unsigned long long* status) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    SortSmem& S = *reinterpret_cast<SortSmem*>(smem_raw);
+    SortSmem<ITEMS>& S = *reinterpret_cast<SortSmem<ITEMS>*>(smem_raw);
+    constexpr int TILE = kSortThreads * ITEMS;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int shift = 8 * pass;
 
+    ETICS_TRACE(0);
+    pdl_launch_dependents();
     if (tid == 0) S.tile = atomicAdd(&tickets[pass], 1u);   // tiles are numbered in the order they start running
 #pragma unroll
-    for (int w = 0; w < kSortWarps; ++w) S.warp_hist[w][tid] = 0;
+    for (int w = 0; w < kSortWarps; ++w) S.warp_hist[w][tid] = make_uint2(0u, 0u);
     __syncthreads();
     const long long tile = S.tile;
-    const long long base = tile * kSortTile + (long long)warp * (32 * kSortItems);
+    const long long base = tile * TILE + (long long)warp * (32 * ITEMS);
+    pdl_wait();
+    ETICS_TRACE(1);
 
-    // ---- load (warp-striped: item i of the warp's 512-key slice sits at base + 32 i + lane) and rank -----------
-    unsigned long long key[kSortItems];
-    unsigned pay[kSortItems];
-    unsigned short rank[kSortItems];
+    // ---- load (warp-striped: item i of the warp's slice sits at base + 32 i + lane) and rank ------------------
+    unsigned long long key[ITEMS];
+    unsigned short rank[ITEMS];
 #pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
+    for (int i = 0; i < ITEMS; ++i) {
         const long long k = base + 32 * i + lane;
-        key[i] = ~0ull;            // padding sorts last in every pass and is never written (position >= N)
-        pay[i] = 0;
-        if (k < N) { key[i] = keys_in[k]; pay[i] = idx_in[k]; }
+        key[i] = (k < N) ? keys_in[k] : ~0ull;   // padding sorts last in every pass and is never written (position >= N)
     }
-    const unsigned lt_mask = (1u << lane) - 1u;
-    unsigned* wh = S.warp_hist[warp];
+    const unsigned hcount = hist[pass * 256 + tid];
+    ETICS_TRACE(2);
+    const unsigned lane_bit = 1u << lane, lt_mask = lane_bit - 1u;
+    uint2* wh = S.warp_hist[warp];
+    // Lanes holding the same digit find each other with eight ballots, one per digit bit.  (Measured on B200, per
+    // SM sub-partition: VOTE 8 cycles; MATCH.ANY 8 cycles per distinct value in the warp, i.e. ~230 for random
+    // digits; a shared-memory atomicOr of lane bits ~1 lane per cycle per SM — both slower than 8 x VOTE.)
 #pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
+    for (int i = 0; i < ITEMS; ++i) {
         const unsigned d = (unsigned)(key[i] >> shift) & 255u;
-        const unsigned peers = __match_any_sync(0xffffffffu, d);
-        const int leader = __ffs(peers) - 1;
-        unsigned prior = 0;
-        if (lane == leader) { prior = wh[d]; wh[d] = prior + __popc(peers); }
-        prior = __shfl_sync(0xffffffffu, prior, leader);
-        rank[i] = (unsigned short)(prior + __popc(peers & lt_mask));
+        unsigned peers = 0xffffffffu;
+#pragma unroll
+        for (int b = 0; b < 8; ++b) {
+            const bool bit = (d >> b) & 1u;
+            const unsigned vote = __ballot_sync(0xffffffffu, bit);
+            peers &= bit ? vote : ~vote;
+        }
+        const unsigned lower = peers & lt_mask;
+        const unsigned prior = wh[d].y;            // every lane of the group reads the count before the leader advances it
+        rank[i] = (unsigned short)(prior + __popc(lower));
+        __syncwarp();
+        if (lower == 0u) wh[d].y = prior + __popc(peers);
         __syncwarp();
     }
+    ETICS_TRACE(3);
     __syncthreads();
 
     // ---- thread d owns digit d: warp offsets, tile count, lookback ---------------------------------------------
     unsigned count = 0;
 #pragma unroll
     for (int w = 0; w < kSortWarps; ++w) {
-        const unsigned t = S.warp_hist[w][tid];
-        S.warp_hist[w][tid] = count;
+        const unsigned t = S.warp_hist[w][tid].y;
+        S.warp_hist[w][tid].y = count;
         count += t;
     }
     const unsigned long long tag_agg = (unsigned long long)(2 * pass + 1) << 56;
@@ -266,42 +305,70 @@ mex_radix_pass_kernel(const unsigned long long* __restrict__ keys_in, const unsi
     volatile unsigned long long* my_status = status + (size_t)tile * 256 + tid;
     if (tile > 0) *my_status = tag_agg | count;
 
-    const unsigned loc = block_exclusive_scan_256(count, S.scan_tmp, nullptr);
-    const unsigned hcount = hist[pass * 256 + tid];
-    const unsigned hbase = block_exclusive_scan_256(hcount, S.scan_tmp, nullptr);   // global start of bucket d
+    const unsigned loc = block_exclusive_scan_256(count, S.scan_tmp);
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) S.warp_hist[w][tid].y += loc;   // -> position inside the tile
+    __syncthreads();
 
+    // ---- reorder inside the tile (stable); keys, ranks and payload leave the registers before the look-back ------
+    {
+        unsigned pay[ITEMS];
+#pragma unroll
+        for (int i = 0; i < ITEMS; ++i) {
+            const long long k = base + 32 * i + lane;
+            pay[i] = (k < N) ? idx_in[k] : 0u;
+        }
+#pragma unroll
+        for (int i = 0; i < ITEMS; ++i) {
+            const unsigned d = (unsigned)(key[i] >> shift) & 255u;
+            const unsigned p = wh[d].y + rank[i];
+            S.keys[p] = key[i];
+            S.idx[p] = pay[i];
+        }
+    }
+    const unsigned hbase = block_exclusive_scan_256(hcount, S.scan_tmp);   // global start of bucket d
+
+    ETICS_TRACE(4);
+    // look back kLookW tiles at a time (independent loads in flight), consume them nearest first
     unsigned long long excl = 0;
     if (tile > 0) {
         long long t = tile - 1;
-        while (true) {
-            const unsigned long long v = *(volatile unsigned long long*)(status + (size_t)t * 256 + tid);
-            const unsigned long long tag = v & ~kCountMask;
-            if (tag == tag_inc) { excl += v & kCountMask; break; }
-            if (tag == tag_agg) { excl += v & kCountMask; --t; }
+        bool done = false;
+        while (!done) {
+            unsigned long long v[kLookW];
+#pragma unroll
+            for (int j = 0; j < kLookW; ++j)
+                v[j] = (t - j >= 0) ? *(volatile unsigned long long*)(status + (size_t)(t - j) * 256 + tid) : tag_inc;
+            int used = kLookW;
+#pragma unroll
+            for (int j = 0; j < kLookW; ++j) {
+                if (!done && used == kLookW) {
+                    const unsigned long long tag = v[j] & ~kCountMask;
+                    if (tag == tag_inc) { excl += v[j] & kCountMask; done = true; }
+                    else if (tag == tag_agg) excl += v[j] & kCountMask;
+                    else used = j;   // not posted yet: poll again from this tile
+                }
+            }
+            t -= used;
+            if (used == 0) __nanosleep(40);
         }
     }
+    ETICS_TRACE(5);
     *my_status = tag_inc | (excl + count);
-    S.local_off[tid] = loc;
     S.gbase[tid] = hbase + (unsigned)excl - loc;
     __syncthreads();
 
-    // ---- reorder inside the tile (stable), then write runs of equal digits ---------------------------------------
+    // ---- write runs of equal digits -------------------------------------------------------------------------------
+    ETICS_TRACE(6);
 #pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
-        const unsigned d = (unsigned)(key[i] >> shift) & 255u;
-        const unsigned p = S.local_off[d] + wh[d] + rank[i];
-        S.keys[p] = key[i];
-        S.idx[p] = pay[i];
-    }
-    __syncthreads();
-#pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
+    for (int i = 0; i < ITEMS; ++i) {
         const unsigned j = i * kSortThreads + tid;
         const unsigned long long kk = S.keys[j];
         const unsigned d = (unsigned)(kk >> shift) & 255u;
         const unsigned g = S.gbase[d] + j;
         if ((long long)g < N) { keys_out[g] = kk; idx_out[g] = S.idx[j]; }
     }
+    ETICS_TRACE(7);
 }
 
 // =========================================================================================================
@@ -651,6 +718,38 @@ mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__
 // ---------------------------------------------------------------------------------------------------------
 // Host side.
 // ---------------------------------------------------------------------------------------------------------
+template <int ITEMS>
+static cudaError_t radix_passes_enqueue(unsigned long long* const* kbuf, unsigned* const* ibuf, unsigned long long* keys_out,
+                                        unsigned* idx_out, long long N, const unsigned* hist, unsigned* tickets,
+                                        unsigned long long* status, cudaStream_t st) {
+    auto kern = mex_radix_pass_kernel<ITEMS>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem<ITEMS>));
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    constexpr int TILE = kSortThreads * ITEMS;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)((N + TILE - 1) / TILE));
+    cfg.blockDim = dim3(kSortThreads);
+    cfg.dynamicSmemBytes = sizeof(SortSmem<ITEMS>);
+    cfg.stream = st;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    for (int pass = 0; pass < kSortPasses; ++pass) {
+        const bool last = pass == kSortPasses - 1;
+        cudaError_t e = cudaLaunchKernelEx(&cfg, kern, (const unsigned long long*)kbuf[pass & 1], (const unsigned*)ibuf[pass & 1],
+                                           last ? keys_out : kbuf[(pass + 1) & 1], last ? idx_out : ibuf[(pass + 1) & 1],
+                                           N, pass, hist, tickets, status);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
 static cudaError_t mex_sort_enqueue(const double* pos, long long N, const MexLayout& L, char* ws,
                                     unsigned long long* keys_out, unsigned* idx_out, cudaStream_t st,
                                     cudaEvent_t ev_keygen = nullptr) {
@@ -669,20 +768,9 @@ static cudaError_t mex_sort_enqueue(const double* pos, long long N, const MexLay
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (ev_keygen) cudaEventRecord(ev_keygen, st);
-    static bool attr_set = false;
-    if (!attr_set) {
-        e = cudaFuncSetAttribute(mex_radix_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
-    for (int pass = 0; pass < kSortPasses; ++pass) {
-        const bool last = pass == kSortPasses - 1;
-        mex_radix_pass_kernel<<<(unsigned)L.sort_tiles, kSortThreads, sizeof(SortSmem), st>>>(
-            kbuf[pass & 1], ibuf[pass & 1], last ? keys_out : kbuf[(pass + 1) & 1], last ? idx_out : ibuf[(pass + 1) & 1],
-            N, pass, hist, tickets, status);
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
-    }
+    e = (N < kSortSmallN) ? radix_passes_enqueue<8>(kbuf, ibuf, keys_out, idx_out, N, hist, tickets, status, st)
+                          : radix_passes_enqueue<16>(kbuf, ibuf, keys_out, idx_out, N, hist, tickets, status, st);
+    if (e != cudaSuccess) return e;
     return cudaSuccess;
 }
 
