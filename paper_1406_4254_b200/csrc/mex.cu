@@ -88,8 +88,8 @@ __host__ __device__ constexpr double mex_dfact(int m) {   // (2m-1)!!
     return v;
 }
 
-// Tile geometry of the scan kernels: kMexThreads chunks of kMexK consecutive sorted particles.
-constexpr int kMexThreads = 128;
+// Tile geometry of the scan kernels: one warp = kMexThreads chunks of kMexK consecutive sorted particles.
+constexpr int kMexThreads = 32;
 constexpr int kMexK = 8;
 constexpr int kMexTile = kMexThreads * kMexK;
 constexpr int kRecFields = 8;   // r, 1/r, cos th, sin th, cos ph, sin ph, mass, (spare)
@@ -530,16 +530,21 @@ __device__ __forceinline__ void mex_eval_particle(const Rec& p, double* __restri
 }
 
 // =========================================================================================================
-// M4 + M5a: chunk aggregates and the tile-level exclusive scans.
-// Shared memory: V[row][kMexThreads + 1] (row = slot of q, then slot of p), SG[row][4] segment totals.
+// M4 + M5a: chunk aggregates and the tile-level exclusive scans.  A tile is ONE WARP: lane = chunk of kMexK
+// consecutive sorted particles (no block barrier anywhere; 1954 independent tiles at N = 10^6 keep every SM
+// sub-partition fed).  Shared memory: V[row][33] (row = slot of q, then slot of p).
+//   1. each lane sums the moments of its chunk in registers (next record prefetched while the current one is used);
+//   2. the sums go to V transposed; lane = row then runs the exclusive scan along the 32 chunks serially
+//      (q rows inside-out, p rows outside-in; the loads do not depend on the running sum, so the chain is 32 DADDs);
+//   3. V is copied to pre[tile][row][lane] (coalesced, immediate offsets), the row totals to tot[row][tile].
 // =========================================================================================================
 constexpr int kVStride = kMexThreads + 1;
-constexpr int kSegs = kMexThreads / 32;
+static_assert(kMexThreads == 32, "the MEX scan kernels use warp-sized tiles");
 
 template <int LMAX, int G>
-__device__ __forceinline__ void mex_aggregate_group(const double* __restrict__ rec_tile, double* V, double* SG,
-                                                    double* __restrict__ pre, double* __restrict__ tot,
-                                                    long long chunks, long long tiles, long long tile) {
+__device__ __forceinline__ void mex_aggregate_group(const double* __restrict__ rec_tile, double* V,
+                                                    double* __restrict__ pre_tile, double* __restrict__ tot,
+                                                    long long tiles, long long tile) {
     constexpr int NS = mex_group_slots(LMAX, G);
     constexpr int RB = mex_row_base(LMAX, G);
     constexpr int ROWS = 2 * NS;
@@ -547,136 +552,156 @@ __device__ __forceinline__ void mex_aggregate_group(const double* __restrict__ r
     double q[NS], pq[NS];
 #pragma unroll
     for (int s = 0; s < NS; ++s) { q[s] = 0.0; pq[s] = 0.0; }
+    Rec p = load_rec(rec_tile, 0, c);
 #pragma unroll 1
     for (int k = 0; k < kMexK; ++k) {
-        const Rec p = load_rec(rec_tile, k, c);
+        const Rec nx = load_rec(rec_tile, (k + 1 < kMexK) ? k + 1 : k, c);
         mex_agg_particle<LMAX, G>(p, q, pq);
+        p = nx;
     }
 #pragma unroll
     for (int s = 0; s < NS; ++s) { V[s * kVStride + c] = q[s]; V[(NS + s) * kVStride + c] = pq[s]; }
-    __syncthreads();
-    // segment-local exclusive scans: q rows inside-out (ascending chunk), p rows outside-in (descending chunk)
-    for (int task = c; task < ROWS * kSegs; task += kMexThreads) {
-        const int seg = task / ROWS, row = task - seg * ROWS;
-        const bool fwd = row < NS;
-        double* v = V + row * kVStride + seg * 32;
+    __syncwarp();
+    for (int row = c; row < ROWS; row += kMexThreads) {
+        double* v = V + row * kVStride;
+        double x[kMexThreads];
+#pragma unroll
+        for (int j = 0; j < kMexThreads; ++j) x[j] = v[j];
         double run = 0.0;
-#pragma unroll 4
-        for (int i = 0; i < 32; ++i) {
-            const int j = fwd ? i : 31 - i;
-            const double t = v[j];
-            v[j] = run;
-            run += t;
+        if (row < NS) {
+#pragma unroll
+            for (int j = 0; j < kMexThreads; ++j) { v[j] = run; run += x[j]; }
+        } else {
+#pragma unroll
+            for (int j = kMexThreads - 1; j >= 0; --j) { v[j] = run; run += x[j]; }
         }
-        SG[row * kSegs + seg] = run;
+        tot[(size_t)(RB + row) * tiles + tile] = run;
     }
-    __syncthreads();
-    const int seg = c >> 5;
-    const long long chunk = tile * kMexThreads + c;
-#pragma unroll 4
-    for (int row = 0; row < ROWS; ++row) {
-        const bool fwd = row < NS;
-        double off = 0.0;
-        if (fwd) { for (int s = 0; s < seg; ++s) off += SG[row * kSegs + s]; }
-        else     { for (int s = kSegs - 1; s > seg; --s) off += SG[row * kSegs + s]; }
-        pre[(size_t)(RB + row) * chunks + chunk] = off + V[row * kVStride + c];
-    }
-    if (c < ROWS) {
-        double t = 0.0;
-        const bool fwd = c < NS;
-        if (fwd) { for (int s = 0; s < kSegs; ++s) t += SG[c * kSegs + s]; }
-        else     { for (int s = kSegs - 1; s >= 0; --s) t += SG[c * kSegs + s]; }
-        tot[(size_t)(RB + c) * tiles + tile] = t;
-    }
-    __syncthreads();
+    __syncwarp();
+#pragma unroll
+    for (int row = 0; row < ROWS; ++row) pre_tile[(RB + row) * kMexThreads + c] = V[row * kVStride + c];
+    __syncwarp();
 }
 
 template <int LMAX>
 __global__ void __launch_bounds__(kMexThreads)
-mex_aggregate_kernel(const double* __restrict__ rec, double* __restrict__ pre, double* __restrict__ tot,
-                     long long chunks, long long tiles) {
-    extern __shared__ __align__(16) double smem_d[];
+mex_aggregate_kernel(const double* __restrict__ rec, double* __restrict__ pre, double* __restrict__ tot, long long tiles) {
     constexpr int MAXROWS = 2 * mex_max_group_slots(LMAX);
-    double* V = smem_d;
-    double* SG = smem_d + MAXROWS * kVStride;
+    __shared__ double V[MAXROWS * kVStride];
     const long long tile = blockIdx.x;
     const double* rec_tile = rec + (size_t)tile * kRecFields * kMexTile;
+    double* pre_tile = pre + (size_t)tile * mex_total_rows(LMAX) * kMexThreads;
     constexpr int NG = mex_num_groups(LMAX);
-    mex_aggregate_group<LMAX, 0>(rec_tile, V, SG, pre, tot, chunks, tiles, tile);
-    if constexpr (NG > 1) mex_aggregate_group<LMAX, 1>(rec_tile, V, SG, pre, tot, chunks, tiles, tile);
-    if constexpr (NG > 2) mex_aggregate_group<LMAX, 2>(rec_tile, V, SG, pre, tot, chunks, tiles, tile);
-    if constexpr (NG > 3) mex_aggregate_group<LMAX, 3>(rec_tile, V, SG, pre, tot, chunks, tiles, tile);
+    mex_aggregate_group<LMAX, 0>(rec_tile, V, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 1) mex_aggregate_group<LMAX, 1>(rec_tile, V, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 2) mex_aggregate_group<LMAX, 2>(rec_tile, V, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 3) mex_aggregate_group<LMAX, 3>(rec_tile, V, pre_tile, tot, tiles, tile);
 }
 
 // =========================================================================================================
-// M5b: exclusive scan of the tile totals, one block per row, fixed order.  Rows [rb, rb+ns) of a group run
-// forward (q), rows [rb+ns, rb+2ns) backward (p).
+// M5b: exclusive scan of the tile totals tot[row][tile], one block per row, fixed order.  Rows [rb, rb+ns) of a
+// group run forward (q), rows [rb+ns, rb+2ns) backward (p).  256 tiles per step: coalesced load, warp-shuffle
+// scan, carry to the next step.
 // =========================================================================================================
 struct RowDirs { int ng; int rb[4]; int ns[4]; };
+constexpr int kTileScanThreads = 256;
+constexpr int kTileScanItems = 8;   // consecutive scan-order positions per thread and step
 
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(kTileScanThreads)
 mex_tilescan_kernel(double* __restrict__ tot, long long tiles, RowDirs rd) {
-    __shared__ double sums[256];
-    const int row = blockIdx.x, t = threadIdx.x;
+    __shared__ double wsum[kTileScanThreads / 32];
+    const int row = blockIdx.x, t = threadIdx.x, lane = t & 31, warp = t >> 5;
     bool fwd = true;
     for (int g = 0; g < rd.ng; ++g)
         if (row >= rd.rb[g] && row < rd.rb[g] + 2 * rd.ns[g]) fwd = row < rd.rb[g] + rd.ns[g];
     double* v = tot + (size_t)row * tiles;
-    const long long seg = (tiles + 255) / 256;
-    const long long j0 = (long long)t * seg, j1 = (j0 + seg < tiles) ? j0 + seg : tiles;   // scan-order positions
-    double local = 0.0;
-    for (long long j = j0; j < j1; ++j) local += v[fwd ? j : tiles - 1 - j];
-    sums[t] = local;
-    __syncthreads();
-    double run = 0.0;
-    for (int u = 0; u < t; ++u) run += sums[u];
-    for (long long j = j0; j < j1; ++j) {
-        const long long i = fwd ? j : tiles - 1 - j;
-        const double x = v[i];
-        v[i] = run;
-        run += x;
+    double carry = 0.0;
+    for (long long base = 0; base < tiles; base += kTileScanThreads * kTileScanItems) {
+        const long long j0 = base + (long long)t * kTileScanItems;   // first scan-order position of this thread
+        double x[kTileScanItems];
+#pragma unroll
+        for (int e = 0; e < kTileScanItems; ++e) {
+            const long long j = j0 + e;
+            x[e] = (j < tiles) ? v[fwd ? j : tiles - 1 - j] : 0.0;
+        }
+        double local = 0.0;
+#pragma unroll
+        for (int e = 0; e < kTileScanItems; ++e) local += x[e];
+        double inc = local;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const double y = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += y;
+        }
+        if (lane == 31) wsum[warp] = inc;
+        double exc = __shfl_up_sync(0xffffffffu, inc, 1);
+        if (lane == 0) exc = 0.0;
+        __syncthreads();
+        double woff = 0.0, total = 0.0;
+#pragma unroll
+        for (int w = 0; w < kTileScanThreads / 32; ++w) {
+            const double s = wsum[w];
+            if (w < warp) woff += s;
+            total += s;
+        }
+        __syncthreads();
+        double run = carry + (woff + exc);
+#pragma unroll
+        for (int e = 0; e < kTileScanItems; ++e) {
+            const long long j = j0 + e;
+            if (j < tiles) v[fwd ? j : tiles - 1 - j] = run;
+            run += x[e];
+        }
+        carry += total;
     }
 }
 
 // =========================================================================================================
 // M5c + M6 + M7: walk, evaluate, transform, scatter.
-// Shared memory: out[k][4][thread] (Phi, a_r, a_theta, a_phi of the thread's K particles).
+// Shared memory: out[k][4][lane] (Phi, a_r, a_theta, a_phi of the lane's K particles; lane-private columns).
 // =========================================================================================================
 template <int LMAX, int G>
 __device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ rec_tile, double* sOut,
-                                                   const double* __restrict__ pre, const double* __restrict__ tot,
-                                                   long long chunks, long long tiles, long long tile) {
+                                                   const double* __restrict__ pre_tile, const double* __restrict__ tot,
+                                                   long long tiles, long long tile) {
     constexpr int NS = mex_group_slots(LMAX, G);
     constexpr int RB = mex_row_base(LMAX, G);
     const int c = threadIdx.x;
-    const long long chunk = tile * kMexThreads + c;
     double s[NS];
     // inside-out: q
 #pragma unroll
-    for (int i = 0; i < NS; ++i) s[i] = pre[(size_t)(RB + i) * chunks + chunk] + tot[(size_t)(RB + i) * tiles + tile];
+    for (int i = 0; i < NS; ++i) s[i] = pre_tile[(RB + i) * kMexThreads + c] + tot[(size_t)(RB + i) * tiles + tile];
+    {
+        Rec p = load_rec(rec_tile, 0, c);
 #pragma unroll 1
-    for (int k = 0; k < kMexK; ++k) {
-        const Rec p = load_rec(rec_tile, k, c);
-        double o[4];
+        for (int k = 0; k < kMexK; ++k) {
+            const Rec nx = load_rec(rec_tile, (k + 1 < kMexK) ? k + 1 : k, c);
+            double o[4];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) o[j] = sOut[(k * 4 + j) * kMexThreads + c];
-        mex_eval_particle<LMAX, G, true>(p, s, o);
+            for (int j = 0; j < 4; ++j) o[j] = sOut[(k * 4 + j) * kMexThreads + c];
+            mex_eval_particle<LMAX, G, true>(p, s, o);
 #pragma unroll
-        for (int j = 0; j < 4; ++j) sOut[(k * 4 + j) * kMexThreads + c] = o[j];
+            for (int j = 0; j < 4; ++j) sOut[(k * 4 + j) * kMexThreads + c] = o[j];
+            p = nx;
+        }
     }
     // outside-in: p
 #pragma unroll
     for (int i = 0; i < NS; ++i)
-        s[i] = pre[(size_t)(RB + NS + i) * chunks + chunk] + tot[(size_t)(RB + NS + i) * tiles + tile];
+        s[i] = pre_tile[(RB + NS + i) * kMexThreads + c] + tot[(size_t)(RB + NS + i) * tiles + tile];
+    {
+        Rec p = load_rec(rec_tile, kMexK - 1, c);
 #pragma unroll 1
-    for (int k = kMexK - 1; k >= 0; --k) {
-        const Rec p = load_rec(rec_tile, k, c);
-        double o[4];
+        for (int k = kMexK - 1; k >= 0; --k) {
+            const Rec nx = load_rec(rec_tile, (k > 0) ? k - 1 : 0, c);
+            double o[4];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) o[j] = sOut[(k * 4 + j) * kMexThreads + c];
-        mex_eval_particle<LMAX, G, false>(p, s, o);
+            for (int j = 0; j < 4; ++j) o[j] = sOut[(k * 4 + j) * kMexThreads + c];
+            mex_eval_particle<LMAX, G, false>(p, s, o);
 #pragma unroll
-        for (int j = 0; j < 4; ++j) sOut[(k * 4 + j) * kMexThreads + c] = o[j];
+            for (int j = 0; j < 4; ++j) sOut[(k * 4 + j) * kMexThreads + c] = o[j];
+            p = nx;
+        }
     }
 }
 
@@ -684,19 +709,19 @@ template <int LMAX>
 __global__ void __launch_bounds__(kMexThreads)
 mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__ idxT,
                     const double* __restrict__ pre, const double* __restrict__ tot,
-                    long long chunks, long long tiles, long long N,
-                    double* __restrict__ acc, double* __restrict__ pot) {
+                    long long tiles, long long N, double* __restrict__ acc, double* __restrict__ pot) {
     __shared__ double sOut[kMexK * 4 * kMexThreads];
     const long long tile = blockIdx.x;
     const int c = threadIdx.x;
     const double* rec_tile = rec + (size_t)tile * kRecFields * kMexTile;
+    const double* pre_tile = pre + (size_t)tile * mex_total_rows(LMAX) * kMexThreads;
 #pragma unroll
-    for (int i = 0; i < kMexK * 4; ++i) sOut[i * kMexThreads + c] = 0.0;   // thread-private column: no barrier needed
+    for (int i = 0; i < kMexK * 4; ++i) sOut[i * kMexThreads + c] = 0.0;   // lane-private column: no barrier needed
     constexpr int NG = mex_num_groups(LMAX);
-    mex_evaluate_group<LMAX, 0>(rec_tile, sOut, pre, tot, chunks, tiles, tile);
-    if constexpr (NG > 1) mex_evaluate_group<LMAX, 1>(rec_tile, sOut, pre, tot, chunks, tiles, tile);
-    if constexpr (NG > 2) mex_evaluate_group<LMAX, 2>(rec_tile, sOut, pre, tot, chunks, tiles, tile);
-    if constexpr (NG > 3) mex_evaluate_group<LMAX, 3>(rec_tile, sOut, pre, tot, chunks, tiles, tile);
+    mex_evaluate_group<LMAX, 0>(rec_tile, sOut, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 1) mex_evaluate_group<LMAX, 1>(rec_tile, sOut, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 2) mex_evaluate_group<LMAX, 2>(rec_tile, sOut, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 3) mex_evaluate_group<LMAX, 3>(rec_tile, sOut, pre_tile, tot, tiles, tile);
 #pragma unroll 1
     for (int k = 0; k < kMexK; ++k) {
         const long long p = tile * kMexTile + (long long)c * kMexK + k;
@@ -787,23 +812,18 @@ static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, d
     const unsigned* idxT = reinterpret_cast<const unsigned*>(ws + L.off_idxT);
     double* pre = reinterpret_cast<double*>(ws + L.off_pre);
     double* tot = reinterpret_cast<double*>(ws + L.off_tot);
-    constexpr int MAXROWS = 2 * mex_max_group_slots(LMAX);
-    const size_t smem = (size_t)(MAXROWS * kVStride + MAXROWS * kSegs) * sizeof(double);
-    auto agg = mex_aggregate_kernel<LMAX>;
-    cudaError_t e = cudaFuncSetAttribute(agg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    agg<<<(unsigned)L.tiles, kMexThreads, smem, st>>>(rec, pre, tot, L.chunks, L.tiles);
-    e = cudaGetLastError();
+    mex_aggregate_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(rec, pre, tot, L.tiles);
+    cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[4], st);
     RowDirs rd{};
     rd.ng = mex_num_groups(LMAX);
     for (int g = 0; g < rd.ng; ++g) { rd.rb[g] = mex_row_base(LMAX, g); rd.ns[g] = mex_group_slots(LMAX, g); }
-    mex_tilescan_kernel<<<mex_total_rows(LMAX), 256, 0, st>>>(tot, L.tiles, rd);
+    mex_tilescan_kernel<<<mex_total_rows(LMAX), kTileScanThreads, 0, st>>>(tot, L.tiles, rd);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[5], st);
-    mex_evaluate_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(rec, idxT, pre, tot, L.chunks, L.tiles, N, acc, pot);
+    mex_evaluate_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(rec, idxT, pre, tot, L.tiles, N, acc, pot);
     e = cudaGetLastError();
     if (ev) cudaEventRecord(ev[6], st);
     return e;
