@@ -130,6 +130,26 @@ class ClockSampler:
         return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
+def max_over_ranks(x: float, device) -> float:
+    """Max of a per-rank scalar over all ranks (identity at world size 1): the timing rule for N > 1."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_seed(rank: int) -> int:
+    """Replicas only: rank r draws its own particle set from seed r."""
+    return int(rank)
+
+
+def whole_job_value(world: int, n_per_rank: int, ms_per_step: float) -> float:
+    """Particles per second over all replicas: every rank pushed n_per_rank particles through each step."""
+    return world * n_per_rank / (ms_per_step * 1e-3)
+
+
 def physical_gpu_index(local_rank: int) -> int:
     vis = os.environ.get("CUDA_VISIBLE_DEVICES")
     if vis:
@@ -220,7 +240,7 @@ def run_ours(args):
     E.etics_init()
 
     desc, model, N, axes, scf, mex_lmax = WORKLOADS[args.workload]
-    pos_np, mass_np = W.particles(model, N, seed=rank, axes=axes)     # one replica per rank, own particle set
+    pos_np, mass_np = W.particles(model, N, seed=replica_seed(rank), axes=axes)   # one replica per rank, own particle set
     pos = torch.from_numpy(pos_np).cuda()
     mass = torch.from_numpy(mass_np).cuda()
     acc = torch.empty((3, N), dtype=torch.float64, device="cuda")
@@ -287,11 +307,8 @@ def run_ours(args):
         ms = timed(step, args.steps, 0)
         barrier()
         wall = time.perf_counter() - wall0
-    total_ms = torch.tensor([float(np.sum(ms))], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
-    ms_per_step = float(total_ms.item()) / args.steps
-    value = world * N / (ms_per_step * 1e-3)
+    ms_per_step = max_over_ranks(float(np.sum(ms)), "cuda") / args.steps
+    value = whole_job_value(world, N, ms_per_step)
 
     # ---- end to end through the host-buffer C-ABI calls ----------------------------------------------------------
     e2e_steps = max(3, min(args.steps, 20))
@@ -315,10 +332,7 @@ def run_ours(args):
             E.etics_mex_full_host(pos_h, mass_h, mex_lmax, acc_h, pot_h, scr_mex)
 
     e2e_ms = timed(e2e_step, e2e_steps, 2)
-    e2e_total = torch.tensor([float(np.sum(e2e_ms))], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(e2e_total, op=dist.ReduceOp.MAX)
-    e2e_value = world * N / (float(e2e_total.item()) / e2e_steps * 1e-3)
+    e2e_value = whole_job_value(world, N, max_over_ranks(float(np.sum(e2e_ms)), "cuda") / e2e_steps)
     if scf is not None:
         del scr_scf
     if mex_lmax is not None:
