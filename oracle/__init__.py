@@ -36,6 +36,7 @@ def lib():
         L.oracle_scf_force.argtypes = [_dp, C.c_longlong, C.c_int, C.c_int, _dp, _dp, _dp, _dp, C.c_int]
         L.oracle_mex_sort.argtypes = [_dp, C.c_longlong, C.POINTER(C.c_ulonglong), C.POINTER(C.c_uint)]
         L.oracle_mex_force.argtypes = [_dp, _dp, C.c_longlong, C.c_int, _dp, _dp, C.POINTER(C.c_uint)]
+        L.oracle_mex_force_at.argtypes = [_dp, _dp, C.c_longlong, C.c_int, C.POINTER(C.c_longlong), C.c_int, _dp, _dp, C.c_int]
         L.oracle_num_threads.argtypes = [C.c_int]
         _lib = L
     return _lib
@@ -137,3 +138,18 @@ def mex_force(pos, mass, lmax: int, return_perm: bool = False):
     if rc != 0:
         raise ValueError(f"oracle_mex_force failed: {rc}")
     return (acc, pot, perm) if return_perm else (acc, pot)
+
+
+def mex_force_at(pos, mass, lmax: int, sample_idx, threads: int = 0):
+    """MEX potential/acceleration of the sampled particles straight from eqs. 11-12 (no sort); (3,S), (S)."""
+    pos = _f64(pos); mass = _f64(mass)
+    n = mass.shape[0]
+    assert pos.shape == (3, n)
+    idx = np.ascontiguousarray(np.asarray(sample_idx, dtype=np.int64))
+    s = idx.shape[0]
+    acc = np.empty((3, s)); pot = np.empty(s)
+    rc = lib().oracle_mex_force_at(_p(pos), _p(mass), n, lmax, idx.ctypes.data_as(C.POINTER(C.c_longlong)), s,
+                                   _p(acc), _p(pot), threads)
+    if rc != 0:
+        raise ValueError(f"oracle_mex_force_at failed: {rc}")
+    return acc, pot

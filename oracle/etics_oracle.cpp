@@ -425,4 +425,119 @@ int oracle_mex_force(const double* pos, const double* mass, long long N, int lma
     return 0;
 }
 
+// ---------------------------------------------------------------------------------------------
+// MEX force at a SAMPLE of particles, straight from the definition — no sort, no streaming carry.
+// For sample particle i, eqs. (11)–(12) PAPER.md:120-123 are sums over "every j strictly interior"
+// and "every j strictly exterior", where (readings G7, G8) j is interior to i iff
+// (key_j, j) < (key_i, i) lexicographically, key = bits of r^2 with the pinned rounding.  So:
+//   1. the S samples are ordered by (key, index);
+//   2. every particle j (in index order, any order would do) is classified by b = number of samples
+//      that are strictly interior to j (0..S).  j is exterior to samples[0..b), and interior to
+//      samples[b'..S) with b' = b, or b + 1 when j is itself samples[b] (no self term);
+//      its exterior-type moment m_j r_j^-(l+1) P_lm {cos,sin} is added to bin pbin[b], its
+//      interior-type moment m_j r_j^l P_lm {cos,sin} to bin qbin[b'];
+//   3. q(sample t) = sum_{b' <= t} qbin[b'],  p(sample t) = sum_{b > t} pbin[b];
+//   4. Phi, a_r, a_theta, a_phi from the full expressions of the header comment above
+//      (Q = q r^-(l+1) + p r^l, R = -(l+1) q r^-(l+2) + l p r^(l-1)), then spherical -> Cartesian.
+// Used by the full-size GPU parity tests (N = 10^8), where the streaming sweep above would take
+// minutes, and pinned against it at small N (tests/test_oracle_pins_mex.py).  OpenMP over j with
+// thread-private bins combined in thread order; Neumaier sums throughout.
+// acc_out is (3,S), pot_out (S), in the order of sample_idx.
+// ---------------------------------------------------------------------------------------------
+int oracle_mex_force_at(const double* pos, const double* mass, long long N, int lmax,
+                        const long long* sample_idx, int S, double* acc_out, double* pot_out, int threads) {
+    if (N < 1 || N >= (1LL << 31) || lmax < 0 || S < 1) return -1;
+    const int L = num_lm(lmax);
+    const double *X = pos, *Y = pos + N, *Z = pos + 2 * N;
+    auto key_of = [&](long long k) {
+        double t = X[k] * X[k];
+        t = std::fma(Y[k], Y[k], t);
+        t = std::fma(Z[k], Z[k], t);
+        uint64_t u; std::memcpy(&u, &t, 8);
+        return u;
+    };
+    for (int s = 0; s < S; ++s) if (sample_idx[s] < 0 || sample_idx[s] >= N) return -1;
+    // 1. samples in (key, index) order; `where[t]` = position in sample_idx of the t-th sample
+    std::vector<std::pair<uint64_t, long long>> so(S);
+    std::vector<int> where(S);
+    std::iota(where.begin(), where.end(), 0);
+    std::sort(where.begin(), where.end(), [&](int a, int b) {
+        return std::make_pair(key_of(sample_idx[a]), sample_idx[a]) < std::make_pair(key_of(sample_idx[b]), sample_idx[b]);
+    });
+    for (int t = 0; t < S; ++t) so[t] = std::make_pair(key_of(sample_idx[where[t]]), sample_idx[where[t]]);
+    for (int t = 1; t < S; ++t) if (so[t] == so[t - 1]) return -2;   // duplicate sample indices
+
+    threads = resolve_threads(threads);
+    const size_t binsz = (size_t)(S + 1) * L;
+    // per thread: qbin cos, qbin sin, pbin cos, pbin sin
+    std::vector<std::vector<Neumaier>> bins(threads, std::vector<Neumaier>(4 * binsz));
+#pragma omp parallel num_threads(threads)
+    {
+#ifdef _OPENMP
+        const int tid = omp_get_thread_num();
+#else
+        const int tid = 0;
+#endif
+        Neumaier* qc = bins[tid].data();
+        Neumaier* qs = qc + binsz;
+        Neumaier* pc = qs + binsz;
+        Neumaier* ps = pc + binsz;
+        std::vector<double> P(L), dP(L), U(L), cm(lmax + 1), sm(lmax + 1);
+#pragma omp for schedule(static)
+        for (long long j = 0; j < N; ++j) {
+            const std::pair<uint64_t, long long> me(key_of(j), j);
+            const int b = (int)(std::lower_bound(so.begin(), so.end(), me) - so.begin());   // samples strictly interior to j
+            const int bq = (b < S && so[b] == me) ? b + 1 : b;
+            Geom g = geometry(X[j], Y[j], Z[j]);
+            legendre_table(lmax, g.ct, g.st, P.data(), dP.data(), U.data());
+            trig_table(lmax, g.cp, g.sp, cm.data(), sm.data());
+            for (int l = 0; l <= lmax; ++l) {
+                const double mq = mass[j] * std::pow(g.r, l), mp = mass[j] * std::pow(g.r, -(l + 1));
+                for (int m = 0; m <= l; ++m) {
+                    const int i = lm_index(l, m);
+                    if (bq <= S - 1) { qc[(size_t)bq * L + i].add(mq * P[i] * cm[m]); qs[(size_t)bq * L + i].add(mq * P[i] * sm[m]); }
+                    if (b >= 1) { pc[(size_t)b * L + i].add(mp * P[i] * cm[m]); ps[(size_t)b * L + i].add(mp * P[i] * sm[m]); }
+                }
+            }
+        }
+    }
+    // combine threads in thread order
+    std::vector<Neumaier> tot(4 * binsz);
+    for (int t = 0; t < threads; ++t)
+        for (size_t i = 0; i < 4 * binsz; ++i) { tot[i].add(bins[t][i].s); tot[i].add(bins[t][i].c); }
+    const Neumaier *qc = tot.data(), *qs = qc + binsz, *pc = qs + binsz, *ps = pc + binsz;
+
+    std::vector<double> P(L), dP(L), U(L), cm(lmax + 1), sm(lmax + 1);
+    for (int t = 0; t < S; ++t) {
+        // 3. exclusive sums of sample t
+        std::vector<Neumaier> Qc(L), Qs(L), Pc(L), Ps(L);
+        for (int b = 0; b <= t; ++b) for (int i = 0; i < L; ++i) { Qc[i].add(qc[(size_t)b * L + i].value()); Qs[i].add(qs[(size_t)b * L + i].value()); }
+        for (int b = S; b > t; --b) for (int i = 0; i < L; ++i) { Pc[i].add(pc[(size_t)b * L + i].value()); Ps[i].add(ps[(size_t)b * L + i].value()); }
+        // 4. evaluate
+        const long long k = so[t].second;
+        Geom g = geometry(X[k], Y[k], Z[k]);
+        legendre_table(lmax, g.ct, g.st, P.data(), dP.data(), U.data());
+        trig_table(lmax, g.cp, g.sp, cm.data(), sm.data());
+        double sp = 0.0, sr = 0.0, st = 0.0, sf = 0.0;
+        for (int l = 0; l <= lmax; ++l) {
+            const double ri = std::pow(g.r, -(l + 1)), rl = std::pow(g.r, l);
+            const double dri = -(l + 1) * std::pow(g.r, -(l + 2)), drl = (l == 0) ? 0.0 : l * std::pow(g.r, l - 1);
+            for (int m = 0; m <= l; ++m) {
+                const int i = lm_index(l, m);
+                const double w = w_lm(l, m);
+                const double Qcv = Qc[i].value() * ri + Pc[i].value() * rl, Qsv = Qs[i].value() * ri + Ps[i].value() * rl;
+                const double Rcv = Qc[i].value() * dri + Pc[i].value() * drl, Rsv = Qs[i].value() * dri + Ps[i].value() * drl;
+                sp += w * P[i] * (Qcv * cm[m] + Qsv * sm[m]);
+                sr += w * P[i] * (Rcv * cm[m] + Rsv * sm[m]);
+                st += w * dP[i] * (Qcv * cm[m] + Qsv * sm[m]);
+                sf += w * U[i] * m * (-Qcv * sm[m] + Qsv * cm[m]);
+            }
+        }
+        const int o = where[t];
+        pot_out[o] = -sp;
+        to_cartesian(g, sr, st / g.r, sf / g.r, &acc_out[o], &acc_out[S + o], &acc_out[2 * S + o]);
+    }
+    return 0;
+}
+
 }  // extern "C"

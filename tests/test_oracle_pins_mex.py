@@ -204,3 +204,29 @@ def test_mex_empty_interior_and_two_particles():
     a, p = oracle.mex_force(pos, mass, 40)
     da, dp = _direct_sum(pos, mass)
     assert np.allclose(p, dp, rtol=1e-12) and np.allclose(a, da, rtol=1e-11, atol=1e-13)
+
+
+@pytest.mark.parametrize("lmax,threads", [(0, 1), (6, 1), (8, 3)])
+def test_mex_force_at_is_the_definition_and_matches_the_streaming_sweep(lmax, threads):
+    """oracle.mex_force_at evaluates eqs. 11-12 for sampled particles straight from their definition (no sort, no
+    carried running sum); the streaming oracle must agree with it on every sampled particle, including tied radii,
+    the innermost/outermost particles and on-axis ones.  Also pinned to the pairwise series (P11) directly."""
+    rng = np.random.default_rng(5)
+    n = 3000
+    pos, mass = W.particles("plummer", n, seed=3)
+    pos[:, 11] = -pos[:, 10]                    # exact tie: 10 is interior to 11
+    pos[:, 12] = [0.0, 0.0, 0.5]
+    mass = mass * rng.uniform(0.5, 1.5, size=n)
+    acc, pot, perm = oracle.mex_force(pos, mass, lmax, return_perm=True)
+    idx = np.unique(np.concatenate([[10, 11, 12, perm[0], perm[1], perm[-1], perm[-2]], rng.integers(0, n, 40)]))
+    rng.shuffle(idx)                            # sample order must not matter
+    acc_s, pot_s = oracle.mex_force_at(pos, mass, lmax, idx, threads=threads)
+    assert np.allclose(pot_s, pot[idx], rtol=1e-13, atol=0)
+    assert np.allclose(acc_s, acc[:, idx], rtol=1e-12, atol=1e-13 * np.abs(acc).max())
+    rank = np.empty(n, dtype=np.int64); rank[perm] = np.arange(n)
+    for s in (0, 1, 2):
+        i = int(idx[s])
+        ref = _pairwise_series_potential(pos[:, i], i, pos, mass, rank, lmax)
+        assert pot_s[s] == pytest.approx(float(ref), rel=1e-12)
+    with pytest.raises(ValueError):
+        oracle.mex_force_at(pos, mass, lmax, [1, 1])
