@@ -68,9 +68,9 @@ def flops_mex_evaluate(lmax):
     return 54 * num_lm(lmax) + 70
 
 
-BYTES_KEYGEN = 24 + 12          # read pos, write key + index
+BYTES_KEYGEN = 32 + 12 + 32     # read pos + mass, write key + index and the packed (x,y,z,m) record
 BYTES_RADIX_PASS = 24           # read key+index, write key+index
-BYTES_GATHER = 4 + 32 + 32      # read index, random read of (x,y,z,m), write the sorted record
+BYTES_GATHER = 4 + 32 + 56 + 4  # read index, one 32-byte sector of (x,y,z,m), write the geometry record + index
 BYTES_SCATTER = 32              # acc + pot at the original index
 
 

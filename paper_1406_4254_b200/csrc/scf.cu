@@ -33,9 +33,20 @@ cudaError_t scf_init_constants() { return etics_upload_constants(); }
 //   (1/sin th) dPhi/dphi += f_l sum_m m U_lm F_m,   U_lm = P_lm / sin(theta) from its own recurrence
 // =========================================================================================================
 constexpr int kEvalThreads = 128;
+#ifndef ETICS_EVAL_MONIC_GEG
+#define ETICS_EVAL_MONIC_GEG 0
+#endif
+#ifndef ETICS_EVAL_MINBLOCKS
+#define ETICS_EVAL_MINBLOCKS 4
+#endif
+
+// gamma_lm of the monic Legendre recurrence q_l = ct q_{l-1} - gamma_lm q_{l-2} (column m, l >= m+2)
+__host__ __device__ constexpr double leg_gamma_c(int l, int m) {
+    return (l >= m + 2) ? double((l + m - 1) * (l - 1 - m)) / double((2 * l - 1) * (2 * l - 3)) : 0.0;
+}
 
 template <int LMAX>
-__global__ void __launch_bounds__(kEvalThreads)
+__global__ void __launch_bounds__(kEvalThreads, LMAX <= 6 ? ETICS_EVAL_MINBLOCKS : 1)
 scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
                 const double* __restrict__ A, const double* __restrict__ B,
                 double* __restrict__ acc, double* __restrict__ pot) {
@@ -47,7 +58,13 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
         int l = 0;
         while (lm_index(l + 1, 0) <= j) ++l;
         const int m = j - lm_index(l, 0);
-        s_tab[n1 * lm_index(l, 0) + n * (l + 1) + m] = make_double2(A[g], B[g]);
+        // monic recurrences below: C_n = g_n Q_n, P_lm = h_lm q_lm; the scales ride on the coefficients
+#if ETICS_EVAL_MONIC_GEG
+        const double sc = c_basis.geg_scale[l][n] * c_basis.leg_scale[l][m];
+#else
+        const double sc = c_basis.leg_scale[l][m];
+#endif
+        s_tab[n1 * lm_index(l, 0) + n * (l + 1) + m] = make_double2(A[g] * sc, B[g] * sc);
     }
     __syncthreads();
 
@@ -55,12 +72,19 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
     if (k >= N) return;
     const Geom g = geometry(pos[k], pos[N + k], pos[2 * N + k]);
 
-    double cm[LMAX + 1], sm[LMAX + 1];
-    cm[0] = 1.0; sm[0] = 0.0;
+    // cos(m phi), sin(m phi): parked in lane-private shared-memory columns while the n loops run, so that the
+    // 4 (l+1) running sums of a level and the two previous angular rows have the registers to themselves
+    double* s_trig = reinterpret_cast<double*>(s_tab + n1 * L) + threadIdx.x;
+    {
+        double c = 1.0, sn = 0.0;
 #pragma unroll
-    for (int m = 1; m <= LMAX; ++m) {
-        cm[m] = fma(cm[m - 1], g.cp, -sm[m - 1] * g.sp);
-        sm[m] = fma(sm[m - 1], g.cp, cm[m - 1] * g.sp);
+        for (int m = 1; m <= LMAX; ++m) {
+            const double c2 = fma(c, g.cp, -sn * g.sp);
+            sn = fma(sn, g.cp, c * g.sp);
+            c = c2;
+            s_trig[(2 * m) * kEvalThreads] = c;
+            s_trig[(2 * m + 1) * kEvalThreads] = sn;
+        }
     }
 
     const double u = __drcp_rn(1.0 + g.r);
@@ -83,24 +107,16 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
             U0[0] = g.ct; U0[1] = 1.0;
         } else {
 #pragma unroll
-            for (int m = 0; m <= l - 2; ++m) {
-                const double a = double(2 * l - 1) / double(l - m), b = double(l + m - 1) / double(l - m);
-                U0[m] = fma(a * g.ct, U1[m], -b * U2[m]);
-            }
-            U0[l - 1] = double(2 * l - 1) * g.ct * U1[l - 1];
-            U0[l] = double(2 * l - 1) * g.st * U1[l - 1];
+            for (int m = 0; m <= l - 2; ++m) U0[m] = fma(g.ct, U1[m], -leg_gamma_c(l, m) * U2[m]);
+            U0[l - 1] = g.ct * U1[l - 1];
+            U0[l] = g.st * U1[l - 1];
         }
-        double Pm[LMAX + 2];
-        Pm[0] = U0[0];
-#pragma unroll
-        for (int m = 1; m <= l; ++m) Pm[m] = g.st * U0[m];
-        Pm[l + 1] = 0.0;
-
         // ---- radial sums over n -----------------------------------------------------------------------
         double sa[LMAX + 1], sad[LMAX + 1], sb[LMAX + 1], sbd[LMAX + 1];
 #pragma unroll
         for (int m = 0; m <= l; ++m) { sa[m] = 0.0; sad[m] = 0.0; sb[m] = 0.0; sbd[m] = 0.0; }
-        double C = 1.0, Cm = 0.0, D = 0.0, Dm = 0.0;
+        double C = 1.0, Cm = 0.0, D = 0.0, Dm = 0.0;   // monic Q_n, Q_{n-1}, dQ_n/dxi, dQ_{n-1}/dxi
+        const double* __restrict__ beta = c_basis.geg_beta[l];
         for (int n = 0; n < n1; ++n) {
 #pragma unroll
             for (int m = 0; m <= l; ++m) {
@@ -112,28 +128,46 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
                     sbd[m] = fma(ab.y, D, sbd[m]);
                 }
             }
+            // Q_{n+1} = xi Q_n - beta_{n+1} Q_{n-1};  Q'_{n+1} = xi Q'_n + Q_n - beta_{n+1} Q'_{n-1}
+#if ETICS_EVAL_MONIC_GEG
+            const double nb = -beta[n + 1];
+            const double Cn = fma(xi, C, nb * Cm);
+            const double Dn = fma(xi, D, fma(nb, Dm, C));
+#else
+            (void)beta;
             const double a = c_basis.geg_a[l][n + 1], b = c_basis.geg_b[l][n + 1];
             const double ax = a * xi;
             const double Cn = fma(ax, C, -b * Cm);
             const double Dn = fma(ax, D, fma(a, C, -b * Dm));
+#endif
             Cm = C; C = Cn; Dm = D; D = Dn;
         }
         tl += n1 * (l + 1);
 
-        // ---- combine the level ------------------------------------------------------------------------
+        // ---- combine the level (P_lm = st U_lm; dP_lm/dtheta = l ct U_lm - (l+m) U_{l-1,m}, dP_l0/dtheta = -st U_l1:
+        //      same-column forms, no cancellation near the poles) -------------------------------------------------
         double lv_p = 0.0, lv_r = 0.0, lv_t = 0.0, lv_f = 0.0;
+        const double lct = double(l) * g.ct;
 #pragma unroll
         for (int m = 0; m <= l; ++m) {
-            const double Ea = fma(sa[m], cm[m], sb[m] * sm[m]);
-            const double Ed = fma(sad[m], cm[m], sbd[m] * sm[m]);
-            double dP;
-            if (m == 0) dP = -Pm[1];
-            else dP = fma(0.5 * double((l + m) * (l - m + 1)), Pm[m - 1], -0.5 * Pm[m + 1]);
-            lv_p = fma(Pm[m], Ea, lv_p);
-            lv_r = fma(Pm[m], Ed, lv_r);
+            const double cmm = (m == 0) ? 1.0 : s_trig[(2 * m) * kEvalThreads];
+            const double smm = (m == 0) ? 0.0 : s_trig[(2 * m + 1) * kEvalThreads];
+            const double Ea = (m == 0) ? sa[0] : fma(sa[m], cmm, sb[m] * smm);
+            const double Ed = (m == 0) ? sad[0] : fma(sad[m], cmm, sbd[m] * smm);
+            double P, dP;
+            if (m == 0) {
+                P = U0[0];
+                dP = (l >= 1) ? -(double(l) * g.st) * U0[1] : 0.0;   // -P_l1 / h_l0, h_l1 / h_l0 = l
+            } else {
+                P = g.st * U0[m];
+                // in monic terms U_{l-1,m} / h_lm = q_{l-1,m} (l-m)/(2l-1)
+                dP = (m < l) ? fma(lct, U0[m], -(double((l + m) * (l - m)) / double(2 * l - 1)) * U1[m]) : lct * U0[m];
+            }
+            lv_p = fma(P, Ea, lv_p);
+            lv_r = fma(P, Ed, lv_r);
             lv_t = fma(dP, Ea, lv_t);
             if (m > 0) {
-                const double Fa = fma(sb[m], cm[m], -sa[m] * sm[m]);
+                const double Fa = fma(sb[m], cmm, -sa[m] * smm);
                 lv_f = fma(double(m) * U0[m], Fa, lv_f);
             }
         }
@@ -263,10 +297,6 @@ __device__ __forceinline__ void acc_unit_level(const double* __restrict__ F, con
     }
 }
 
-// gamma_lm of the monic Legendre recurrence q_l = ct q_{l-1} - gamma_lm q_{l-2} (column m, l >= m+2)
-__host__ __device__ constexpr double leg_gamma_c(int l, int m) {
-    return (l >= m + 2) ? double((l + m - 1) * (l - 1 - m)) / double((2 * l - 1) * (2 * l - 3)) : 0.0;
-}
 
 // Phase 1, one m-column of one particle (compile-time M): monic q_l = ct q_{l-1} - gamma_lm q_{l-2}, q_M = st^M;
 // rows of level l: q_l0 at l^2, (q_lM cos M phi, q_lM sin M phi) at l^2 + 2M - 1, l^2 + 2M.  Fy already points at
@@ -603,7 +633,7 @@ template <int LMAX>
 static cudaError_t launch_eval(const double* pos, long long N, int nmax, const double* A, const double* B,
                                double* acc, double* pot, cudaStream_t st) {
     auto kern = scf_eval_kernel<LMAX>;
-    const size_t smem = (size_t)(nmax + 1) * num_lm(LMAX) * sizeof(double2);
+    const size_t smem = (size_t)(nmax + 1) * num_lm(LMAX) * sizeof(double2) + (size_t)(2 * LMAX + 2) * kEvalThreads * sizeof(double);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const long long blocks = (N + kEvalThreads - 1) / kEvalThreads;
