@@ -272,7 +272,7 @@ def run_ours(args):
         if mex_lmax is not None:
             mex_force()
 
-    launches_per_step = (3 if scf is not None else 0) + (13 if mex_lmax is not None else 0)
+    launches_per_step = (3 if scf is not None else 0) + (14 if mex_lmax is not None else 0)
 
     def timed(fn, iters, warmup):
         """Per-iteration CUDA-event times (ms) with an L2 flush before every iteration (outside the events)."""
@@ -381,7 +381,7 @@ def run_ours(args):
         add("mex_gather", st["gather"], "hbm", N * BYTES_GATHER)
         add("mex_aggregate", st["aggregate"], "alu", N * flops_mex_aggregate(mex_lmax))
         add("mex_tilescan", st["tilescan"], "hbm", 0)
-        add("mex_evaluate", st["evaluate"], "alu", N * flops_mex_evaluate(mex_lmax))
+        add("mex_evaluate(+unpack)", st["evaluate"], "alu", N * flops_mex_evaluate(mex_lmax), 2)
     dom = max((k for k in kernels if kernels[k]["achieved"] > 0), key=lambda k: kernels[k]["ms"])
     d = kernels[dom]
     roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"], "unit": d["unit"],

@@ -32,22 +32,32 @@ namespace etics {
 cudaError_t mex_init_constants() { return cudaSuccess; }   // every MEX constant is a compile-time literal
 
 // =========================================================================================================
-// Column groups.  Column m holds the pairs (l,m), l = m..LMAX.  kGroupOf[LMAX][m] assigns columns to groups of
-// at most 17 pairs, balanced by hand.
+// Column groups.  Column m holds the pairs (l,m), l = m..LMAX; a group is a set of whole columns.
 // =========================================================================================================
+// Column -> group tables: greedy balanced partition (columns in descending count of running sums, each to the least
+// loaded group) for a target of 28 running sums per direction and group; generated offline, fixed at compile time.
+// (Targets of 18 and 13 — 126 registers/thread, 16 resident warps per SM instead of 12 — were measured: no gain.)
+constexpr int kMexMaxGroups = 8;
+#define ETICS_MEX_NG_INIT {1, 1, 1, 1, 1, 2, 2, 3, 3, 4, 5}
+#define ETICS_MEX_GOF_INIT { \
+    {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, \
+    {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, \
+    {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, \
+    {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, \
+    {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, \
+    {1, 0, 1, 0, 1, 0, 0, 0, 0, 0, 0}, \
+    {0, 0, 1, 1, 1, 0, 0, 0, 0, 0, 0}, \
+    {2, 0, 1, 2, 1, 0, 2, 0, 0, 0, 0}, \
+    {1, 0, 1, 2, 2, 0, 2, 1, 0, 0, 0}, \
+    {3, 0, 1, 2, 3, 2, 1, 0, 3, 0, 0}, \
+    {4, 0, 1, 2, 3, 4, 3, 2, 1, 0, 4}}
 __host__ __device__ constexpr int mex_num_groups(int lmax) {
-    return lmax <= 4 ? 1 : lmax <= 6 ? 2 : lmax <= 8 ? 3 : 4;
+    constexpr int t[ETICS_MAX_LMAX + 1] = ETICS_MEX_NG_INIT;
+    return t[lmax];
 }
 __host__ __device__ constexpr int mex_group_of(int lmax, int m) {
-    switch (lmax) {
-        case 5: return m <= 1 ? 0 : 1;                                            // 11 | 10
-        case 6: return (m <= 1 || m == 6) ? 0 : 1;                                // 14 | 14
-        case 7: return (m == 0 || m == 3) ? 0 : (m == 1 || m == 4 || m == 7) ? 1 : 2;   // 13 | 12 | 11
-        case 8: return (m == 0 || m == 3) ? 0 : (m == 1 || m == 2) ? 1 : 2;       // 15 | 15 | 15
-        case 9: return (m == 0 || m == 6) ? 0 : (m == 1 || m == 5) ? 1 : (m == 2 || m == 4) ? 2 : 3;   // 14 14 14 13
-        case 10: return (m == 0 || m == 5) ? 0 : (m == 1 || m == 4) ? 1 : (m == 2 || m == 3) ? 2 : 3;  // 17 17 17 15
-        default: return 0;
-    }
+    constexpr int t[ETICS_MAX_LMAX + 1][ETICS_MAX_LMAX + 1] = ETICS_MEX_GOF_INIT;
+    return t[lmax][m];
 }
 // running sums per direction of column m: cos only for m = 0, (cos, sin) otherwise
 __host__ __device__ constexpr int mex_col_slots(int lmax, int m) { return (lmax - m + 1) * (m == 0 ? 1 : 2); }
@@ -102,7 +112,10 @@ constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kSortPasses = 8;
 constexpr int kSortMinTile = kSortThreads * 8;     // the status buffer is sized for the smallest tile
 constexpr int kLookW = 16;                         // tiles inspected per look-back round
-constexpr long long kSortSmallN = 1ll << 22;       // N below this: ITEMS = 8
+constexpr long long kSortSmallN = 1ll << 19;       // N below this: ITEMS = 8.  (At N = 10^6 the whole sort is one wave of
+                                                   // tiles and 54 % of the executed instructions are look-back polls, whose
+                                                   // number grows with tiles^2: 245 tiles of 4096 keys run 8 passes in 137 us,
+                                                   // 489 tiles of 2048 keys in 148 us; profiles/r1b_summary.md.)
 
 struct MexLayout {
     long long N;
@@ -631,6 +644,10 @@ mex_aggregate_kernel(const double* __restrict__ rec, double* __restrict__ pre, d
     if constexpr (NG > 1) mex_aggregate_group<LMAX, 1>(rec_tile, V, pre_tile, tot, tiles, tile);
     if constexpr (NG > 2) mex_aggregate_group<LMAX, 2>(rec_tile, V, pre_tile, tot, tiles, tile);
     if constexpr (NG > 3) mex_aggregate_group<LMAX, 3>(rec_tile, V, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 4) mex_aggregate_group<LMAX, 4>(rec_tile, V, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 5) mex_aggregate_group<LMAX, 5>(rec_tile, V, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 6) mex_aggregate_group<LMAX, 6>(rec_tile, V, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 7) mex_aggregate_group<LMAX, 7>(rec_tile, V, pre_tile, tot, tiles, tile);
 }
 
 // =========================================================================================================
@@ -638,7 +655,7 @@ mex_aggregate_kernel(const double* __restrict__ rec, double* __restrict__ pre, d
 // group run forward (q), rows [rb+ns, rb+2ns) backward (p).  256 tiles per step: coalesced load, warp-shuffle
 // scan, carry to the next step.
 // =========================================================================================================
-struct RowDirs { int ng; int rb[4]; int ns[4]; };
+struct RowDirs { int ng; int rb[kMexMaxGroups]; int ns[kMexMaxGroups]; };
 constexpr int kTileScanThreads = 256;
 constexpr int kTileScanItems = 8;   // consecutive scan-order positions per thread and step
 
@@ -740,11 +757,15 @@ __device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ re
     }
 }
 
+__device__ __forceinline__ void st_global_v4(double* p, double a, double b, double c, double d) {
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+
 template <int LMAX>
 __global__ void __launch_bounds__(kMexThreads)
 mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__ idxT,
                     const double* __restrict__ pre, const double* __restrict__ tot,
-                    long long tiles, long long N, double* __restrict__ acc, double* __restrict__ pot) {
+                    long long tiles, long long N, double* __restrict__ out4) {
     __shared__ double sOut[kMexK * 4 * kMexThreads];
     const long long tile = blockIdx.x;
     const int c = threadIdx.x;
@@ -757,6 +778,10 @@ mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__
     if constexpr (NG > 1) mex_evaluate_group<LMAX, 1>(rec_tile, sOut, pre_tile, tot, tiles, tile);
     if constexpr (NG > 2) mex_evaluate_group<LMAX, 2>(rec_tile, sOut, pre_tile, tot, tiles, tile);
     if constexpr (NG > 3) mex_evaluate_group<LMAX, 3>(rec_tile, sOut, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 4) mex_evaluate_group<LMAX, 4>(rec_tile, sOut, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 5) mex_evaluate_group<LMAX, 5>(rec_tile, sOut, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 6) mex_evaluate_group<LMAX, 6>(rec_tile, sOut, pre_tile, tot, tiles, tile);
+    if constexpr (NG > 7) mex_evaluate_group<LMAX, 7>(rec_tile, sOut, pre_tile, tot, tiles, tile);
 #pragma unroll 1
     for (int k = 0; k < kMexK; ++k) {
         const long long p = tile * kMexTile + (long long)c * kMexK + k;
@@ -768,11 +793,22 @@ mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__
         double ax, ay, az;
         to_cartesian(g, sOut[(k * 4 + 1) * kMexThreads + c], sOut[(k * 4 + 2) * kMexThreads + c],
                      sOut[(k * 4 + 3) * kMexThreads + c], ax, ay, az);
-        acc[i] = ax;
-        acc[N + i] = ay;
-        acc[2 * N + i] = az;
-        pot[i] = sOut[(k * 4 + 0) * kMexThreads + c];
+        // ONE full 32-byte sector per particle at its original index (four 8-byte stores into the SoA outputs cost
+        // 22 us of the kernel's 120 at N = 10^6 and 5 of 22 ms at N = 10^8); mex_unpack_kernel streams it into acc, pot
+        st_global_v4(out4 + 4 * (size_t)i, sOut[(k * 4 + 0) * kMexThreads + c], ax, ay, az);
     }
+}
+
+// (Phi, ax, ay, az) records by original index -> pot (N), acc (3,N).  Streaming: 32 B read + 32 B written per particle.
+__global__ void __launch_bounds__(256)
+mex_unpack_kernel(const double2* __restrict__ out4, long long N, double* __restrict__ acc, double* __restrict__ pot) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double2 a = out4[2 * i], b = out4[2 * i + 1];
+    pot[i] = a.x;
+    acc[i] = a.y;
+    acc[N + i] = b.x;
+    acc[2 * N + i] = b.y;
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -862,7 +898,11 @@ static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, d
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[5], st);
-    mex_evaluate_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(rec, idxT, pre, tot, L.tiles, N, acc, pot);
+    double* out4 = reinterpret_cast<double*>(ws + L.off_pk);   // the packed inputs were consumed by the gather
+    mex_evaluate_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(rec, idxT, pre, tot, L.tiles, N, out4);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    mex_unpack_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(reinterpret_cast<const double2*>(out4), N, acc, pot);
     e = cudaGetLastError();
     if (ev) cudaEventRecord(ev[6], st);
     return e;
