@@ -455,12 +455,29 @@ mex_gather_kernel(const double2* __restrict__ pk, const unsigned* __restrict__ p
 
 // =========================================================================================================
 // Per-particle column arithmetic (eqs. 15–17; real form and weights: DESIGN.md "Readings").
-// Column m, stable l-recurrence (never the paper's eq. 24):
-//   m = 0 : P_0 = 1, P_1 = ct, l P_l = (2l-1) ct P_{l-1} - (l-1) P_{l-2}
-//   m >= 1: U_mm = (2m-1)!! st^(m-1), U_{m+1,m} = (2m+1) ct U_mm, (l-m) U_l = (2l-1) ct U_{l-1} - (l+m-1) U_{l-2},
-//           P_lm = st U_lm   (U_lm = P_lm / sin theta is a polynomial: nothing is divided by sin theta)
-// Same-column derivative: dP_lm/dtheta = l ct U_lm - (l+m) U_{l-1,m} (m >= 1);  dP_l0/dtheta = -st U_l1.
+// Column m, stable l-recurrence (never the paper's eq. 24), in MONIC form so that every step
+// is one multiply and one FMA:
+//   P_lm = h_lm sin(theta) u_lm (m >= 1),  P_l0 = h_l0 u_l0;   h_mm = (2m-1)!!,  h_lm = h_{l-1,m} (2l-1)/(l-m)
+//   u_mm = st^(m-1) (u_00 = 1),  u_{m+1,m} = ct u_mm,  u_lm = ct u_{l-1,m} - gamma_lm u_{l-2,m},
+//   gamma_lm = (l+m-1)(l-1-m) / ((2l-1)(2l-3))
+// (u_lm sin(theta) = P_lm / h_lm; u_lm itself is a polynomial in ct, st: nothing is divided by sin theta.)
+// The running sums carry the weight W_lm = w_lm h_lm^2 (one P from the source particle, one from the target):
+//   S^{c,s}_lm = sum_j W_lm m_j {r_j^l | r_j^-(l+1)} Y_lm(j) {cos, sin}(m phi_j),   Y_lm = st u_lm  (Y_l0 = u_l0)
+// Same-column derivative: (dP_lm/dtheta)/h_lm = l ct u_lm - (l+m)(l-m)/(2l-1) u_{l-1,m}  (m >= 1);
+//                         (dP_l0/dtheta)/h_l0 = -l st u_l1   (h_l1 / h_l0 = l).
 // =========================================================================================================
+__host__ __device__ constexpr double mex_h(int l, int m) {
+    double v = mex_dfact(m);
+    for (int k = m + 1; k <= l; ++k) v = v * double(2 * k - 1) / double(k - m);
+    return v;
+}
+__host__ __device__ constexpr double mex_W(int l, int m) { return mex_w(l, m) * mex_h(l, m) * mex_h(l, m); }
+__host__ __device__ constexpr double mex_gamma(int l, int m) {
+    return (l >= m + 2) ? double((l + m - 1) * (l - 1 - m)) / double((2 * l - 1) * (2 * l - 3)) : 0.0;
+}
+__host__ __device__ constexpr bool mex_in_group(int lmax, int g, int m) { return m <= lmax && mex_group_of(lmax, m) == g; }
+
+// cos(m phi), sin(m phi), st^(m-1) of the columns of group G (the chains run over every m; unused entries vanish)
 template <int LMAX>
 struct Angles {
     double cm[LMAX + 1], sm[LMAX + 1];   // cos m phi, sin m phi
@@ -487,17 +504,18 @@ __device__ __forceinline__ void mex_agg_particle(const Rec& p, double* __restric
     for (int l = 1; l <= LMAX; ++l) { mq[l] = mq[l - 1] * p.r; mp[l] = mp[l - 1] * p.rinv; }
 #pragma unroll
     for (int m = 0; m <= LMAX; ++m) {
-        if (mex_group_of(LMAX, m) != G) continue;
+        if (!mex_in_group(LMAX, G, m)) continue;
         const int sb = mex_slot_base(LMAX, m);
-        double P1 = 0.0, P2 = 0.0;   // P_{l-1,m}, P_{l-2,m}
+        double u1 = 0.0, u2 = 0.0;   // u_{l-1,m}, u_{l-2,m}
 #pragma unroll
         for (int l = m; l <= LMAX; ++l) {
-            double P;
-            if (l == m) P = (m == 0) ? 1.0 : mex_dfact(m) * a.sp1[m] * p.st;
-            else if (l == m + 1) P = double(2 * m + 1) * p.ct * P1;
-            else P = fma(double(2 * l - 1) / double(l - m) * p.ct, P1, -(double(l + m - 1) / double(l - m)) * P2);
-            P2 = P1; P1 = P;
-            const double tq = (mex_w(l, m) * mq[l]) * P, tp = (mex_w(l, m) * mp[l]) * P;
+            double u;
+            if (l == m) u = (m == 0) ? 1.0 : a.sp1[m];
+            else if (l == m + 1) u = p.ct * u1;
+            else u = fma(p.ct, u1, -mex_gamma(l, m) * u2);
+            u2 = u1; u1 = u;
+            const double wy = (m == 0) ? mex_W(l, 0) * u : (mex_W(l, m) * p.st) * u;
+            const double tq = mq[l] * wy, tp = mp[l] * wy;
             if (m == 0) {
                 q[sb + l] += tq;
                 pq[sb + l] += tp;
@@ -514,62 +532,80 @@ __device__ __forceinline__ void mex_agg_particle(const Rec& p, double* __restric
 // direction, THEN add the particle's own moment (exclusive sums, eqs. 11–12).
 //   FWD: s = q (interior), radial factor r^-(l+1), d/dr factor -(l+1)/r;  own moment m r^l
 //   BWD: s = p (exterior), radial factor r^l,      d/dr factor  l/r;      own moment m r^-(l+1)
-// out[0..3] += (Phi, a_r, a_theta, a_phi) contributions.
+// Level by level: the m sums of a level (P, dP/dtheta, U-weighted) are formed first and meet the radial factor
+// once per level.  out[0..3] += (Phi, a_r, a_theta, a_phi) contributions.
 template <int LMAX, int G, bool FWD>
 __device__ __forceinline__ void mex_eval_particle(const Rec& p, double* __restrict__ s, double* __restrict__ out) {
     Angles<LMAX> a;
     a.init(p);
-    double rho[LMAX + 1], mu[LMAX + 1];
-    if (FWD) { rho[0] = p.rinv; mu[0] = p.mass; } else { rho[0] = 1.0; mu[0] = p.mass * p.rinv; }
+    double mcm[LMAX + 1], msm[LMAX + 1];   // m cos(m phi), m sin(m phi): the d/dphi factor rides on the rotation
 #pragma unroll
-    for (int l = 1; l <= LMAX; ++l) {
-        rho[l] = rho[l - 1] * (FWD ? p.rinv : p.r);
-        mu[l] = mu[l - 1] * (FWD ? p.r : p.rinv);
-    }
+    for (int m = 1; m <= LMAX; ++m) { mcm[m] = double(m) * a.cm[m]; msm[m] = double(m) * a.sm[m]; }
+    constexpr bool kAux1 = mex_in_group(LMAX, G, 0) && !mex_in_group(LMAX, G, 1) && LMAX >= 1;   // m = 0 needs u_l1
+    double u1[LMAX + 1], u2[LMAX + 1];     // u_{l-1,m}, u_{l-2,m} per column
+#pragma unroll
+    for (int m = 0; m <= LMAX; ++m) { u1[m] = 0.0; u2[m] = 0.0; }
+    double x1 = 0.0, x2 = 0.0;             // the auxiliary m = 1 column when it lives in another group
+    double rho = FWD ? p.rinv : 1.0;       // r^-(l+1) | r^l
+    double mu = FWD ? p.mass : p.mass * p.rinv;   // m r^l | m r^-(l+1)
     double sP = 0.0, sR = 0.0, sT = 0.0, sF = 0.0;
 #pragma unroll
-    for (int m = 0; m <= LMAX; ++m) {
-        if (mex_group_of(LMAX, m) != G) continue;
-        const int sb = mex_slot_base(LMAX, m);
-        double U1 = 0.0, U2 = 0.0;   // U_{l-1}, U_{l-2} of this column (P for m = 0)
-        double W1 = 0.0, W2 = 0.0;   // m = 0 only: the m = 1 column U_{l-1,1}, U_{l-2,1} for dP_l0/dtheta
+    for (int l = 0; l <= LMAX; ++l) {
+        // ---- the level's u_lm ---------------------------------------------------------------------------
+        double u[LMAX + 1];
 #pragma unroll
-        for (int l = m; l <= LMAX; ++l) {
-            double U;
-            if (l == m) U = (m == 0) ? 1.0 : mex_dfact(m) * a.sp1[m];
-            else if (l == m + 1) U = double(2 * m + 1) * p.ct * U1;
-            else U = fma(double(2 * l - 1) / double(l - m) * p.ct, U1, -(double(l + m - 1) / double(l - m)) * U2);
-            const double kappa = FWD ? -double(l + 1) : double(l);
+        for (int m = 0; m <= l; ++m) {
+            if (!mex_in_group(LMAX, G, m)) continue;
+            if (l == m) u[m] = (m == 0) ? 1.0 : a.sp1[m];
+            else if (l == m + 1) u[m] = p.ct * u1[m];
+            else u[m] = fma(p.ct, u1[m], -mex_gamma(l, m) * u2[m]);
+        }
+        double ul1 = 0.0;                  // u_l1, for dP_l0/dtheta
+        if (mex_in_group(LMAX, G, 0) && l >= 1) {
+            if (kAux1) {
+                const double x = (l == 1) ? 1.0 : (l == 2) ? p.ct * x1 : fma(p.ct, x1, -mex_gamma(l, 1) * x2);
+                x2 = x1; x1 = x;
+                ul1 = x;
+            } else {
+                ul1 = u[1];
+            }
+        }
+        // ---- sums over the group's m at this level, then the own moment ------------------------------------
+        const double lct = double(l) * p.ct;
+        double aP = 0.0, aT = 0.0, aF = 0.0;
+#pragma unroll
+        for (int m = 0; m <= l; ++m) {
+            if (!mex_in_group(LMAX, G, m)) continue;
+            const int sb = mex_slot_base(LMAX, m);
             if (m == 0) {
-                double W = 0.0;   // U_{l,1}
-                if (l == 1) W = 1.0;
-                else if (l == 2) W = 3.0 * p.ct;
-                else if (l > 2) W = fma(double(2 * l - 1) / double(l - 1) * p.ct, W1, -(double(l) / double(l - 1)) * W2);
-                W2 = W1; W1 = W;
-                const double e = rho[l] * s[sb + l];
-                const double ye = U * e;
-                sP += ye;
-                sR = fma(kappa, ye, sR);
-                sT = fma(-p.st * W, e, sT);
-                s[sb + l] = fma(mex_w(l, 0) * mu[l], U, s[sb + l]);
+                const double e = s[sb + l];
+                aP = fma(u[0], e, aP);
+                if (l >= 1) aT = fma(-(double(l) * p.st) * ul1, e, aT);
+                s[sb + l] = fma(mex_W(l, 0) * mu, u[0], e);
             } else {
                 const int i = sb + 2 * (l - m);
                 const double E = fma(s[i], a.cm[m], s[i + 1] * a.sm[m]);
-                const double F = fma(s[i + 1], a.cm[m], -s[i] * a.sm[m]);
-                const double e = rho[l] * E, f = rho[l] * F;
-                const double Y = p.st * U;
-                const double T = fma(double(l) * p.ct, U, -double(l + m) * U1);
-                const double ye = Y * e;
-                sP += ye;
-                sR = fma(kappa, ye, sR);
-                sT = fma(T, e, sT);
-                sF = fma(double(m) * U, f, sF);
-                const double t = (mex_w(l, m) * mu[l]) * Y;
+                const double F = fma(s[i + 1], mcm[m], -s[i] * msm[m]);
+                const double Y = p.st * u[m];
+                const double T = (m < l) ? fma(lct, u[m], -(double((l + m) * (l - m)) / double(2 * l - 1)) * u1[m]) : lct * u[m];
+                aP = fma(Y, E, aP);
+                aT = fma(T, E, aT);
+                aF = fma(u[m], F, aF);
+                const double t = (mex_W(l, m) * mu) * Y;
                 s[i] = fma(t, a.cm[m], s[i]);
                 s[i + 1] = fma(t, a.sm[m], s[i + 1]);
             }
-            U2 = U1; U1 = U;
         }
+        const double pa = rho * aP;
+        sP += pa;
+        sR = fma(FWD ? -double(l + 1) : double(l), pa, sR);
+        sT = fma(rho, aT, sT);
+        sF = fma(rho, aF, sF);
+        rho *= FWD ? p.rinv : p.r;
+        mu *= FWD ? p.r : p.rinv;
+#pragma unroll
+        for (int m = 0; m <= l; ++m)
+            if (mex_in_group(LMAX, G, m)) { u2[m] = u1[m]; u1[m] = u[m]; }
     }
     out[0] -= sP;
     out[1] = fma(p.rinv, sR, out[1]);
