@@ -74,6 +74,16 @@ BYTES_GATHER = 4 + 32 + 56 + 4  # read index, one 32-byte sector of (x,y,z,m), w
 BYTES_SCATTER = 32              # acc + pot at the original index
 
 
+def ncu_traffic(workload):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel, from the committed
+    `ncu --set full` capture of this workload (profiles/traffic_<workload>.json names the capture); {} if none."""
+    path = os.path.join(ROOT, "profiles", f"traffic_{workload}.json")
+    if not os.path.exists(path):
+        return {}
+    with open(path) as f:
+        return json.load(f).get("dram_bytes_per_launch", {})
+
+
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -382,10 +392,13 @@ def run_ours(args):
         add("mex_aggregate", st["aggregate"], "alu", N * flops_mex_aggregate(mex_lmax))
         add("mex_tilescan", st["tilescan"], "hbm", 0)
         add("mex_evaluate(+unpack)", st["evaluate"], "alu", N * flops_mex_evaluate(mex_lmax), 2)
+    traffic = ncu_traffic(args.workload)
+    for k in kernels:
+        kernels[k]["traffic"] = traffic.get(k)
     dom = max((k for k in kernels if kernels[k]["achieved"] > 0), key=lambda k: kernels[k]["ms"])
     d = kernels[dom]
     roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"], "unit": d["unit"],
-                "frac": d["frac"], "traffic": None, "share_of_step": d["ms"] / sum(v["ms"] for v in kernels.values()),
+                "frac": d["frac"], "traffic": d["traffic"], "share_of_step": d["ms"] / sum(v["ms"] for v in kernels.values()),
                 "peak_source": ("148 SMs x 64 fp64 lanes x 2 x sm_max_mhz (DESIGN.md)" if d["bound"] == "alu" else peaks["source"])}
 
     # measured fp64 FMA rate of this GPU (register-resident DFMA chains), for context beside the derived peak
