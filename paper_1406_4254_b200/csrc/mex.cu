@@ -224,7 +224,10 @@ mex_keygen_kernel(const double* __restrict__ pos, const double* __restrict__ mas
 // Ranking: the lanes of a warp that hold the same digit are found with eight ballots (one per digit bit) —
 // the MATCH.ANY instruction iterates over the distinct values of the warp and was the kernel's bottleneck
 // (profiles/r1b_summary.md).  Launched with programmatic stream serialisation: the prologue (ticket, clearing the
-// counters) overlaps the tail of the preceding pass; griddepcontrol.wait orders every read of its output.
+// counters) overlaps the tail of the preceding pass; griddepcontrol.wait orders every read of its output, and those
+// reads are L2-coherent loads (ld.global.cg), never the non-coherent path a const __restrict__ pointer would allow —
+// the block was resident before the producer finished.  (Extending the same launch mode to the other MEX kernels,
+// which read their inputs through the non-coherent path, produced wrong results at N = 2049 and was dropped.)
 // =========================================================================================================
 constexpr unsigned long long kCountMask = (1ull << 56) - 1;
 
@@ -307,9 +310,9 @@ mex_radix_pass_kernel(const unsigned long long* __restrict__ keys_in, const unsi
 #pragma unroll
     for (int i = 0; i < ITEMS; ++i) {
         const long long k = base + 32 * i + lane;
-        key[i] = (k < N) ? keys_in[k] : ~0ull;   // padding sorts last in every pass and is never written (position >= N)
+        key[i] = (k < N) ? __ldcg(keys_in + k) : ~0ull;   // padding sorts last in every pass and is never written (position >= N)
     }
-    const unsigned hcount = hist[pass * 256 + tid];
+    const unsigned hcount = __ldcg(hist + pass * 256 + tid);
     ETICS_TRACE(2);
     const unsigned lane_bit = 1u << lane, lt_mask = lane_bit - 1u;
     uint2* wh = S.warp_hist[warp];
@@ -360,7 +363,7 @@ mex_radix_pass_kernel(const unsigned long long* __restrict__ keys_in, const unsi
 #pragma unroll
         for (int i = 0; i < ITEMS; ++i) {
             const long long k = base + 32 * i + lane;
-            pay[i] = (k < N) ? idx_in[k] : 0u;
+            pay[i] = (k < N) ? __ldcg(idx_in + k) : 0u;
         }
 #pragma unroll
         for (int i = 0; i < ITEMS; ++i) {
