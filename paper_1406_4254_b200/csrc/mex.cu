@@ -111,7 +111,7 @@ constexpr int kSortThreads = 256;
 constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kSortPasses = 8;
 constexpr int kSortMinTile = kSortThreads * 8;     // the status buffer is sized for the smallest tile
-constexpr int kLookW = 16;                         // tiles inspected per look-back round
+constexpr int kLookW = 4;                          // tiles inspected per look-back round (measured 1..32: 4 is best at 1e6 and 1e8)
 constexpr long long kSortSmallN = 1ll << 19;       // N below this: ITEMS = 8.  (At N = 10^6 the whole sort is one wave of
                                                    // tiles and 54 % of the executed instructions are look-back polls, whose
                                                    // number grows with tiles^2: 245 tiles of 4096 keys run 8 passes in 137 us,
