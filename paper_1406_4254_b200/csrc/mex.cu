@@ -640,7 +640,7 @@ __device__ __forceinline__ void mex_aggregate_group(const double* __restrict__ r
 #pragma unroll
     for (int s = 0; s < NS; ++s) { q[s] = 0.0; pq[s] = 0.0; }
     Rec p = load_rec(rec_tile, 0, c);
-#pragma unroll 1
+#pragma unroll(LMAX <= 6 ? 1 : 2)
     for (int k = 0; k < kMexK; ++k) {
         const Rec nx = load_rec(rec_tile, (k + 1 < kMexK) ? k + 1 : k, c);
         mex_agg_particle<LMAX, G>(p, q, pq);
@@ -764,7 +764,7 @@ __device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ re
     for (int i = 0; i < NS; ++i) s[i] = pre_tile[(RB + i) * kMexThreads + c] + tot[(size_t)(RB + i) * tiles + tile];
     {
         Rec p = load_rec(rec_tile, 0, c);
-#pragma unroll 1
+#pragma unroll(LMAX <= 6 ? 1 : 2)   // two particles in flight per walk pay at lmax >= 7 (N = 1e8, lmax 8: 18.0 -> 16.4 ms)
         for (int k = 0; k < kMexK; ++k) {
             const Rec nx = load_rec(rec_tile, (k + 1 < kMexK) ? k + 1 : k, c);
             double o[4];
@@ -782,7 +782,7 @@ __device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ re
         s[i] = pre_tile[(RB + NS + i) * kMexThreads + c] + tot[(size_t)(RB + NS + i) * tiles + tile];
     {
         Rec p = load_rec(rec_tile, kMexK - 1, c);
-#pragma unroll 1
+#pragma unroll(LMAX <= 6 ? 1 : 2)   // two particles in flight per walk pay at lmax >= 7 (N = 1e8, lmax 8: 18.0 -> 16.4 ms)
         for (int k = kMexK - 1; k >= 0; --k) {
             const Rec nx = load_rec(rec_tile, (k > 0) ? k - 1 : 0, c);
             double o[4];
@@ -801,7 +801,7 @@ __device__ __forceinline__ void st_global_v4(double* p, double a, double b, doub
 }
 
 template <int LMAX>
-__global__ void __launch_bounds__(kMexThreads)
+__global__ void __launch_bounds__(kMexThreads, LMAX <= 6 ? 12 : 8)
 mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__ idxT,
                     const double* __restrict__ pre, const double* __restrict__ tot,
                     long long tiles, long long N, double* __restrict__ out4) {

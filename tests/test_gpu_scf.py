@@ -85,6 +85,14 @@ def test_every_lmax(E, lmax):
     check_scf(E, pos, mass, 4, lmax)
 
 
+@pytest.mark.parametrize("lmax", range(0, 8))
+def test_nmax10_every_lmax(E, lmax):
+    """nmax = 10 selects the evaluation kernel with fully unrolled n loops for lmax <= 6 (monic Gegenbauer recurrence,
+    scales folded into the coefficient table); lmax = 7 takes the run-time loop at the same nmax."""
+    pos, mass = W.particles("hernquist", 2777, seed=13, axes=(1.0, 0.7, 0.9))
+    check_scf(E, pos, mass, 10, lmax)
+
+
 @pytest.mark.parametrize("n", [1, 2, 31, 32, 33, 63, 64, 65, 127, 129, 1000, 37889])
 def test_ragged_sizes(E, n):
     """Sizes around the pass (32/64 particles) and block boundaries, including a single particle."""
