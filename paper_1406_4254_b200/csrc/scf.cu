@@ -447,11 +447,14 @@ scf_accumulate_kernel(const double* __restrict__ pos, const double* __restrict__
         phase1(pass + 1);     // reads G[(pass+1)&1] (written before the previous barrier), writes F[(pass+1)&1]
         if (active) {         // reads F[pass&1] (written before the previous barrier)
             const double* F = sF + (size_t)(pass & 1) * fbuf;
+            // single-group tables: code specialised per level (beta_n as immediates).  Multi-group tables run the generic
+            // code for every unit: up to 11 levels x 4 widths of specialised code thrash the instruction cache
+            // ((20,10), N = 1e7: 11.2 -> 9.5 ms with the generic path; (10,6) is the other way round, 132 vs 152 us)
             switch (u.w) {
-                case 1: acc_unit_level<1>(F, g, u, g.rep, my_rep, lane, acc); break;
-                case 2: acc_unit_level<2>(F, g, u, g.rep, my_rep, lane, acc); break;
-                case 3: acc_unit_level<3>(F, g, u, g.rep, my_rep, lane, acc); break;
-                default: acc_unit_level<4>(F, g, u, g.rep, my_rep, lane, acc); break;
+                case 1: if (FULL) acc_unit_level<1>(F, g, u, g.rep, my_rep, lane, acc); else acc_unit_steps<1, -1>(F, g, u, g.rep, my_rep, lane, acc); break;
+                case 2: if (FULL) acc_unit_level<2>(F, g, u, g.rep, my_rep, lane, acc); else acc_unit_steps<2, -1>(F, g, u, g.rep, my_rep, lane, acc); break;
+                case 3: if (FULL) acc_unit_level<3>(F, g, u, g.rep, my_rep, lane, acc); else acc_unit_steps<3, -1>(F, g, u, g.rep, my_rep, lane, acc); break;
+                default: if (FULL) acc_unit_level<4>(F, g, u, g.rep, my_rep, lane, acc); else acc_unit_steps<4, -1>(F, g, u, g.rep, my_rep, lane, acc); break;
             }
         }
         __syncthreads();
