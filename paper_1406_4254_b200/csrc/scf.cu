@@ -116,7 +116,7 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
         for (int m = 0; m <= l; ++m) { sa[m] = 0.0; sad[m] = 0.0; sb[m] = 0.0; sbd[m] = 0.0; }
         double C = 1.0, Cm = 0.0, D = 0.0, Dm = 0.0;   // monic Q_n, Q_{n-1}, dQ_n/dxi, dQ_{n-1}/dxi
         const double* __restrict__ beta = c_basis.geg_beta[l];
-#pragma unroll
+#pragma unroll(N1C == 0 ? 4 : N1C > 16 ? 3 : 32)
         for (int n = 0; n < (N1C > 0 ? N1C : n1); ++n) {
 #pragma unroll
             for (int m = 0; m <= l; ++m) {
@@ -648,8 +648,10 @@ template <int LMAX>
 static cudaError_t launch_eval(const double* pos, long long N, int nmax, const double* A, const double* B,
                                double* acc, double* pot, cudaStream_t st) {
     // nmax = 10 (the paper's cut-off) at lmax <= 6 gets fully unrolled n loops: 166.5 -> 149 us at N = 1e6.
-    // (Unrolling (20,10) as well — 5544 FMAs of straight-line code at 248 registers — was slower: 6.4 -> 8.5 ms at 1e7.)
+    // (20,10) with compile-time nmax and the n loops unrolled by 3: 6.41 -> 6.08 ms at N = 1e7 (fully unrolled — 5544
+    // FMAs of straight-line code — it was slower, 8.5 ms).
     if (LMAX <= 6 && nmax == 10) return launch_eval_n<LMAX, (LMAX <= 6 ? 11 : 0)>(pos, N, nmax, A, B, acc, pot, st);
+    if (LMAX == 10 && nmax == 20) return launch_eval_n<LMAX, (LMAX == 10 ? 21 : 0)>(pos, N, nmax, A, B, acc, pot, st);
     return launch_eval_n<LMAX, 0>(pos, N, nmax, A, B, acc, pot, st);
 }
 
