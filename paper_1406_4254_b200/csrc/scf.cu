@@ -32,9 +32,10 @@ cudaError_t scf_init_constants() { return etics_upload_constants(); }
 //   dPhi/dth   += f_l sum_m dP_lm E_m
 //   (1/sin th) dPhi/dphi += f_l sum_m m U_lm F_m,   U_lm = P_lm / sin(theta) from its own recurrence
 // =========================================================================================================
-constexpr int kEvalThreads = 128;
+// threads per block: 64: 166 us, 128: 148.5, 256: 145.4, 512: 162.6 at (10,6), N = 1e6; (20,10) at N = 1e7: 128: 6.08 ms, 256: 6.45 ms
+__host__ __device__ constexpr int eval_threads(int lmax) { return lmax <= 6 ? 256 : 128; }
 #ifndef ETICS_EVAL_MINBLOCKS
-#define ETICS_EVAL_MINBLOCKS 4
+#define ETICS_EVAL_MINBLOCKS 2
 #endif
 
 // gamma_lm of the monic Legendre recurrence q_l = ct q_{l-1} - gamma_lm q_{l-2} (column m, l >= m+2)
@@ -45,7 +46,7 @@ __host__ __device__ constexpr double leg_gamma_c(int l, int m) {
 // N1C > 0: nmax + 1 known at compile time (the n loops unroll fully and the compiler schedules across them);
 // N1C = 0: run-time nmax.
 template <int LMAX, int N1C>
-__global__ void __launch_bounds__(kEvalThreads, LMAX <= 6 ? ETICS_EVAL_MINBLOCKS : 1)
+__global__ void __launch_bounds__(eval_threads(LMAX), LMAX <= 6 ? ETICS_EVAL_MINBLOCKS : 1)
 scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
                 const double* __restrict__ A, const double* __restrict__ B,
                 double* __restrict__ acc, double* __restrict__ pot) {
@@ -56,6 +57,7 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
     extern __shared__ double2 s_tab[];   // (A,B) pairs, index n1*l(l+1)/2 + n*(l+1) + m
     constexpr int L = num_lm(LMAX);
     const int n1 = N1C > 0 ? N1C : nmax + 1;
+    constexpr int kEvalThreads = eval_threads(LMAX);
     for (int g = threadIdx.x; g < n1 * L; g += kEvalThreads) {
         const int n = g / L, j = g - n * L;
         int l = 0;
@@ -636,6 +638,7 @@ template <int LMAX, int N1C>
 static cudaError_t launch_eval_n(const double* pos, long long N, int nmax, const double* A, const double* B,
                                  double* acc, double* pot, cudaStream_t st) {
     auto kern = scf_eval_kernel<LMAX, N1C>;
+    constexpr int kEvalThreads = eval_threads(LMAX);
     const size_t smem = (size_t)(nmax + 1) * num_lm(LMAX) * sizeof(double2) + (size_t)(2 * LMAX + 2) * kEvalThreads * sizeof(double);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
