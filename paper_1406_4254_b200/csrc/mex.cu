@@ -27,9 +27,18 @@
 // exclusive_scan per (m, re/im, direction), a partial-force kernel; finally a coordinate-transform kernel.
 #include "etics_common.cuh"
 
+// This file is compiled four times (paper_1406_4254_b200/build.py) with ETICS_MEX_PART = 0..3: part 0 holds the sort,
+// the host entry points and the scan kernels for lmax <= 6; parts 1-3 only instantiate the scan kernels for lmax 7-8, 9
+// and 10 — the template instances dominate the compile time and the parts build in parallel.
+#ifndef ETICS_MEX_PART
+#define ETICS_MEX_PART 0
+#endif
+
 namespace etics {
 
+#if ETICS_MEX_PART == 0
 cudaError_t mex_init_constants() { return cudaSuccess; }   // every MEX constant is a compile-time literal
+#endif
 
 // =========================================================================================================
 // Column groups.  Column m holds the pairs (l,m), l = m..LMAX; a group is a set of whole columns.
@@ -157,7 +166,9 @@ static MexLayout make_mex_layout(long long N, int lmax) {
     return L;
 }
 
+#if ETICS_MEX_PART == 0
 size_t mex_workspace(long long N, int lmax) { return make_mex_layout(N, lmax).total; }
+#endif
 
 // =========================================================================================================
 // M1: keys + byte histograms.
@@ -433,7 +444,7 @@ __device__ __forceinline__ Rec load_rec(const double* __restrict__ rec_tile, int
     return p;
 }
 
-__global__ void __launch_bounds__(256)
+static __global__ void __launch_bounds__(256)
 mex_gather_kernel(const double2* __restrict__ pk, const unsigned* __restrict__ perm,
                   long long N, long long tiles, double* __restrict__ rec, unsigned* __restrict__ idxT) {
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -698,7 +709,7 @@ struct RowDirs { int ng; int rb[kMexMaxGroups]; int ns[kMexMaxGroups]; };
 constexpr int kTileScanThreads = 256;
 constexpr int kTileScanItems = 8;   // consecutive scan-order positions per thread and step
 
-__global__ void __launch_bounds__(kTileScanThreads)
+static __global__ void __launch_bounds__(kTileScanThreads)
 mex_tilescan_kernel(double* __restrict__ tot, long long tiles, RowDirs rd) {
     __shared__ double wsum[kTileScanThreads / 32];
     const int row = blockIdx.x, t = threadIdx.x, lane = t & 31, warp = t >> 5;
@@ -839,7 +850,7 @@ mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__
 }
 
 // (Phi, ax, ay, az) records by original index -> pot (N), acc (3,N).  Streaming: 32 B read + 32 B written per particle.
-__global__ void __launch_bounds__(256)
+static __global__ void __launch_bounds__(256)
 mex_unpack_kernel(const double2* __restrict__ out4, long long N, double* __restrict__ acc, double* __restrict__ pot) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
@@ -853,6 +864,7 @@ mex_unpack_kernel(const double2* __restrict__ out4, long long N, double* __restr
 // ---------------------------------------------------------------------------------------------------------
 // Host side.
 // ---------------------------------------------------------------------------------------------------------
+#if ETICS_MEX_PART == 0
 template <int ITEMS>
 static cudaError_t radix_passes_enqueue(unsigned long long* const* kbuf, unsigned* const* ibuf, unsigned long long* keys_out,
                                         unsigned* idx_out, long long N, const unsigned* hist, unsigned* tickets,
@@ -919,6 +931,8 @@ cudaError_t mex_sort_launch(const double* pos, long long N, unsigned long long* 
     return mex_sort_enqueue(pos, nullptr, N, L, static_cast<char*>(ws), keys_sorted, perm, false, st);
 }
 
+#endif   // ETICS_MEX_PART == 0
+
 template <int LMAX>
 static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, double* acc, double* pot, cudaStream_t st,
                                     cudaEvent_t* ev) {
@@ -947,6 +961,45 @@ static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, d
     return e;
 }
 
+// The scan launch sequence of one lmax range per translation unit.
+#define ETICS_SCAN_ARGS const MexLayout &L, char *ws, long long N, int lmax, double *acc, double *pot, cudaStream_t st, cudaEvent_t *ev
+cudaError_t mex_scan_part0(ETICS_SCAN_ARGS);
+cudaError_t mex_scan_part1(ETICS_SCAN_ARGS);
+cudaError_t mex_scan_part2(ETICS_SCAN_ARGS);
+cudaError_t mex_scan_part3(ETICS_SCAN_ARGS);
+#define ETICS_CASE(LM) case LM: return mex_scan_enqueue<LM>(L, ws, N, acc, pot, st, ev);
+#if ETICS_MEX_PART == 0
+cudaError_t mex_scan_part0(ETICS_SCAN_ARGS) {
+    switch (lmax) {
+        ETICS_CASE(0) ETICS_CASE(1) ETICS_CASE(2) ETICS_CASE(3) ETICS_CASE(4) ETICS_CASE(5) ETICS_CASE(6)
+        default: return cudaErrorInvalidValue;
+    }
+}
+#elif ETICS_MEX_PART == 1
+cudaError_t mex_scan_part1(ETICS_SCAN_ARGS) {
+    switch (lmax) {
+        ETICS_CASE(7) ETICS_CASE(8)
+        default: return cudaErrorInvalidValue;
+    }
+}
+#elif ETICS_MEX_PART == 2
+cudaError_t mex_scan_part2(ETICS_SCAN_ARGS) {
+    switch (lmax) {
+        ETICS_CASE(9)
+        default: return cudaErrorInvalidValue;
+    }
+}
+#else
+cudaError_t mex_scan_part3(ETICS_SCAN_ARGS) {
+    switch (lmax) {
+        ETICS_CASE(10)
+        default: return cudaErrorInvalidValue;
+    }
+}
+#endif
+#undef ETICS_CASE
+
+#if ETICS_MEX_PART == 0
 // ev (optional): 7 events recorded at: start, after keygen, after the radix passes, after gather, after aggregate,
 // after tilescan, after evaluate.
 static cudaError_t mex_force_enqueue(const double* pos, const double* mass, long long N, int lmax,
@@ -966,13 +1019,10 @@ static cudaError_t mex_force_enqueue(const double* pos, const double* mass, long
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[3], st);
-    switch (lmax) {
-#define ETICS_CASE(LM) case LM: return mex_scan_enqueue<LM>(L, ws, N, acc, pot, st, ev);
-        ETICS_CASE(0) ETICS_CASE(1) ETICS_CASE(2) ETICS_CASE(3) ETICS_CASE(4) ETICS_CASE(5)
-        ETICS_CASE(6) ETICS_CASE(7) ETICS_CASE(8) ETICS_CASE(9) ETICS_CASE(10)
-#undef ETICS_CASE
-        default: return cudaErrorInvalidValue;
-    }
+    if (lmax <= 6) return mex_scan_part0(L, ws, N, lmax, acc, pot, st, ev);
+    if (lmax <= 8) return mex_scan_part1(L, ws, N, lmax, acc, pot, st, ev);
+    if (lmax == 9) return mex_scan_part2(L, ws, N, lmax, acc, pot, st, ev);
+    return mex_scan_part3(L, ws, N, lmax, acc, pot, st, ev);
 }
 
 cudaError_t mex_force_launch(const double* pos, const double* mass, long long N, int lmax,
@@ -992,5 +1042,7 @@ cudaError_t mex_force_timed(const double* pos, const double* mass, long long N, 
     for (auto& x : ev) cudaEventDestroy(x);
     return e;
 }
+
+#endif   // ETICS_MEX_PART == 0
 
 }  // namespace etics
