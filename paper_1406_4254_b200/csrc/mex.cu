@@ -292,8 +292,11 @@ __device__ __forceinline__ unsigned block_exclusive_scan_256(unsigned v, unsigne
     return woff + inc - v;
 }
 
-template <int ITEMS>
-__global__ void __launch_bounds__(kSortThreads, ITEMS <= 8 ? 4 : 3)
+// MINB = resident blocks per SM the register allocation is sized for.  A sort whose tiles all fit in one wave at two
+// blocks per SM (N ~ 10^6) runs faster with 123 registers and no spills (8 passes: 125 -> 117 us); a large sort wants the
+// third resident block (N = 10^8: 6.3 ms against 7.2 ms).
+template <int ITEMS, int MINB>
+__global__ void __launch_bounds__(kSortThreads, MINB)
 mex_radix_pass_kernel(const unsigned long long* __restrict__ keys_in, const unsigned* __restrict__ idx_in,
                       unsigned long long* __restrict__ keys_out, unsigned* __restrict__ idx_out,
                       long long N, int pass, const unsigned* __restrict__ hist, unsigned* __restrict__ tickets,
@@ -865,11 +868,11 @@ mex_unpack_kernel(const double2* __restrict__ out4, long long N, double* __restr
 // Host side.
 // ---------------------------------------------------------------------------------------------------------
 #if ETICS_MEX_PART == 0
-template <int ITEMS>
+template <int ITEMS, int MINB>
 static cudaError_t radix_passes_enqueue(unsigned long long* const* kbuf, unsigned* const* ibuf, unsigned long long* keys_out,
                                         unsigned* idx_out, long long N, const unsigned* hist, unsigned* tickets,
                                         unsigned long long* status, cudaStream_t st) {
-    auto kern = mex_radix_pass_kernel<ITEMS>;
+    auto kern = mex_radix_pass_kernel<ITEMS, MINB>;
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem<ITEMS>));
@@ -919,8 +922,15 @@ static cudaError_t mex_sort_enqueue(const double* pos, const double* mass, long 
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (ev_keygen) cudaEventRecord(ev_keygen, st);
-    e = (N < kSortSmallN) ? radix_passes_enqueue<8>(kbuf, ibuf, keys_out, idx_out, N, hist, tickets, status, st)
-                          : radix_passes_enqueue<16>(kbuf, ibuf, keys_out, idx_out, N, hist, tickets, status, st);
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 148;
+    }
+    const long long tiles16 = (N + kSortThreads * 16 - 1) / (kSortThreads * 16);
+    if (N < kSortSmallN) e = radix_passes_enqueue<8, 4>(kbuf, ibuf, keys_out, idx_out, N, hist, tickets, status, st);
+    else if (tiles16 <= 2ll * sms) e = radix_passes_enqueue<16, 2>(kbuf, ibuf, keys_out, idx_out, N, hist, tickets, status, st);
+    else e = radix_passes_enqueue<16, 3>(kbuf, ibuf, keys_out, idx_out, N, hist, tickets, status, st);
     if (e != cudaSuccess) return e;
     return cudaSuccess;
 }
