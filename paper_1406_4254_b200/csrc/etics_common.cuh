@@ -7,6 +7,7 @@
 
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cmath>
 #include <cstddef>
 #include <cstdint>
@@ -105,22 +106,51 @@ inline void fill_basis_constants(BasisConstants& c) {
         }
 }
 
+// One-time set-up per DEVICE (function attributes and __constant__ copies belong to a device; one process may
+// drive several GPUs, and several host threads may call in): run(f) calls f once for the current device.
+struct DeviceOnce {
+    std::mutex mu;
+    std::atomic<bool> done[64] = {};
+    template <class F>
+    cudaError_t run(F&& f) {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        if (dev < 0 || dev >= 64) return f();
+        if (done[dev].load(std::memory_order_acquire)) return cudaSuccess;
+        std::lock_guard<std::mutex> lock(mu);
+        if (done[dev].load(std::memory_order_relaxed)) return cudaSuccess;
+        e = f();
+        if (e == cudaSuccess) done[dev].store(true, std::memory_order_release);
+        return e;
+    }
+};
+
+// SM count of the current device (148 when no device is present, so that size queries work on a CPU-only box).
+inline int device_sm_count() {
+    static std::atomic<int> sms[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+    int v = sms[dev].load(std::memory_order_relaxed);
+    if (v == 0) {
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) v = 148;
+        sms[dev].store(v, std::memory_order_relaxed);
+    }
+    return v;
+}
+
 // One __constant__ copy per translation unit (no relocatable device code needed).
 #define ETICS_DEFINE_CONSTANTS()                                                                     \
     static __constant__ etics::BasisConstants c_basis;                                               \
     static cudaError_t etics_upload_constants() {                                                    \
-        static std::mutex mu;                                                                        \
-        static bool done[64] = {};                                                                   \
-        int dev = 0;                                                                                 \
-        cudaError_t e = cudaGetDevice(&dev);                                                         \
-        if (e != cudaSuccess) return e;                                                              \
-        std::lock_guard<std::mutex> lock(mu);                                                        \
-        if (dev >= 0 && dev < 64 && done[dev]) return cudaSuccess;                                   \
-        static etics::BasisConstants host;                                                           \
-        etics::fill_basis_constants(host);                                                           \
-        e = cudaMemcpyToSymbol(c_basis, &host, sizeof(host));                                        \
-        if (e == cudaSuccess && dev >= 0 && dev < 64) done[dev] = true;                              \
-        return e;                                                                                    \
+        static etics::DeviceOnce once;                                                               \
+        return once.run([] {                                                                         \
+            etics::BasisConstants* host = new etics::BasisConstants;                                 \
+            etics::fill_basis_constants(*host);                                                      \
+            cudaError_t e = cudaMemcpyToSymbol(c_basis, host, sizeof(*host));                        \
+            delete host;                                                                             \
+            return e;                                                                                \
+        });                                                                                          \
     }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -25,7 +25,7 @@
 // What the paper did instead (prior art, §3.2): Thrust merge sort of particle structs, a cache
 // kernel, then per l: a summand kernel writing q_lm, p_lm of every particle to global memory, one Thrust
 // exclusive_scan per (m, re/im, direction), a partial-force kernel; finally a coordinate-transform kernel.
-#include "etics_common.cuh"
+#include "mex_common.cuh"
 
 // This file is compiled four times (paper_1406_4254_b200/build.py) with ETICS_MEX_PART = 0..3: part 0 holds the sort,
 // the host entry points and the scan kernels for lmax <= 6; parts 1-3 only instantiate the scan kernels for lmax 7-8, 9
@@ -37,7 +37,7 @@
 namespace etics {
 
 #if ETICS_MEX_PART == 0
-cudaError_t mex_init_constants() { return cudaSuccess; }   // every MEX constant is a compile-time literal
+cudaError_t mex_init_constants() { return mex_sort_init_device(); }   // every MEX constant is a compile-time literal; per-device function attributes
 #endif
 
 // =========================================================================================================
@@ -107,56 +107,26 @@ __host__ __device__ constexpr double mex_dfact(int m) {   // (2m-1)!!
     return v;
 }
 
-// Tile geometry of the scan kernels: one warp = kMexThreads chunks of kMexK consecutive sorted particles.
-constexpr int kMexThreads = 32;
-constexpr int kMexK = 8;
-constexpr int kMexTile = kMexThreads * kMexK;
-constexpr int kRecFields = 8;   // r, 1/r, cos th, sin th, cos ph, sin ph, mass, (spare)
-
-// Radix sort geometry: 256 threads (thread d owns digit d in the offset phase), ITEMS keys per thread.
-// ITEMS = 8 (2048-key tiles): more tiles and a shorter ranking chain per tile — the passes of a small sort are
-// latency bound; ITEMS = 16 (4096-key tiles): longer runs of equal digits per tile for the large sorts.
-constexpr int kSortThreads = 256;
-constexpr int kSortWarps = kSortThreads / 32;
-constexpr int kSortPasses = 8;
-constexpr int kSortMinTile = kSortThreads * 8;     // the status buffer is sized for the smallest tile
-constexpr int kLookW = 4;                          // tiles inspected per look-back round (measured 1..32: 4 is best at 1e6 and 1e8)
-constexpr long long kSortSmallN = 1ll << 19;       // N below this: ITEMS = 8.  (At N = 10^6 the whole sort is one wave of
-                                                   // tiles and 54 % of the executed instructions are look-back polls, whose
-                                                   // number grows with tiles^2: 245 tiles of 4096 keys run 8 passes in 137 us,
-                                                   // 489 tiles of 2048 keys in 148 us; profiles/r1b_summary.md.)
-
-struct MexLayout {
-    long long N;
-    int lmax;
-    long long sort_tiles, tiles, chunks;   // chunks = tiles * kMexThreads
-    int rows;
-    size_t off_zero, zero_bytes;           // [hist 8x256 u32 | tickets 8 u32 | status sort_tiles*256 u64]
-    size_t off_hist, off_ticket, off_status;
-    size_t off_keysA, off_keysB, off_idxA, off_idxB;
-    size_t off_pk;                         // packed (x, y, z, m) by original index: one 32-byte sector per gather
-    size_t off_rec, off_idxT, off_pre, off_tot;
-    size_t total;
-};
-
-static MexLayout make_mex_layout(long long N, int lmax) {
+#if ETICS_MEX_PART == 0
+MexLayout make_mex_layout(long long N, int lmax) {
     MexLayout L{};
     L.N = N; L.lmax = lmax;
-    L.sort_tiles = (N + kSortMinTile - 1) / kSortMinTile;
+    L.sort_rows = (N + kSortMinTile - 1) / kSortMinTile;
     L.tiles = (N + kMexTile - 1) / kMexTile;
     L.chunks = L.tiles * kMexThreads;
     L.rows = mex_total_rows(lmax);
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += round_up(bytes, 256); return at; };
     L.off_zero = o;
-    L.off_hist = take((size_t)kSortPasses * 256 * sizeof(unsigned));
-    L.off_ticket = take(64);
-    L.off_status = take((size_t)L.sort_tiles * 256 * sizeof(unsigned long long));
+    L.off_hdr = take(sizeof(SortHeader));
+    L.off_hist = take((size_t)kSortMaxPasses * kSortBins * sizeof(unsigned));
+    L.off_status = take((size_t)kSortMaxPasses * L.sort_rows * kSortBins * sizeof(unsigned));
     L.zero_bytes = o - L.off_zero;
-    L.off_keysA = take((size_t)N * 8);
-    L.off_keysB = take((size_t)N * 8);
-    L.off_idxA = take((size_t)N * 4);
-    L.off_idxB = take((size_t)N * 4);
+    L.off_keys = take((size_t)N * 8);
+    L.off_wordsA = take((size_t)N * 8);
+    L.off_wordsB = take((size_t)N * 8);
+    L.off_perm = take((size_t)N * 4);
+    L.off_itmp = take((size_t)N * 4);
     L.off_pk = take((size_t)N * 32);
     L.off_rec = take((size_t)L.tiles * kRecFields * kMexTile * 8);
     L.off_idxT = take((size_t)L.tiles * kMexTile * 4);
@@ -166,271 +136,8 @@ static MexLayout make_mex_layout(long long N, int lmax) {
     return L;
 }
 
-#if ETICS_MEX_PART == 0
 size_t mex_workspace(long long N, int lmax) { return make_mex_layout(N, lmax).total; }
 #endif
-
-// =========================================================================================================
-// M1: keys + byte histograms.
-// =========================================================================================================
-__device__ __forceinline__ unsigned long long mex_key(double x, double y, double z) {
-    double t = __dmul_rn(x, x);
-    t = __fma_rn(y, y, t);
-    t = __fma_rn(z, z, t);
-    return (unsigned long long)__double_as_longlong(t);   // r^2 >= 0: the bit pattern is monotone in r^2
-}
-
-// PACK: also write (x, y, z, m) of particle k as one 32-byte record pk[k], so that the gather after the sort reads
-// one aligned sector per particle instead of four (at N = 10^8 the four-array gather ran at 11 % of HBM).
-// Four particles per thread and iteration with every load issued before the first use; the histogram of the top
-// byte (sign + high exponent bits: a handful of distinct values in any warp) is aggregated per warp with
-// match.any before touching shared memory, the other seven go straight to shared-memory atomics.
-constexpr int kKeygenItems = 4;
-
-template <bool PACK>
-__global__ void __launch_bounds__(256)
-mex_keygen_kernel(const double* __restrict__ pos, const double* __restrict__ mass, long long N,
-                  unsigned long long* __restrict__ keys, unsigned* __restrict__ idx, unsigned* __restrict__ hist,
-                  double2* __restrict__ pk) {
-    __shared__ unsigned sh[kSortPasses * 256];
-    for (int i = threadIdx.x; i < kSortPasses * 256; i += 256) sh[i] = 0;
-    __syncthreads();
-    const int lane = threadIdx.x & 31;
-    const long long stride = (long long)gridDim.x * 256 * kKeygenItems;
-    for (long long base = (long long)blockIdx.x * 256 * kKeygenItems; base < N; base += stride) {
-        double x[kKeygenItems], y[kKeygenItems], z[kKeygenItems], mk[kKeygenItems];
-#pragma unroll
-        for (int j = 0; j < kKeygenItems; ++j) {
-            const long long k = base + j * 256 + threadIdx.x;
-            const bool ok = k < N;
-            x[j] = ok ? pos[k] : 0.0; y[j] = ok ? pos[N + k] : 0.0; z[j] = ok ? pos[2 * N + k] : 0.0;
-            if (PACK) mk[j] = ok ? mass[k] : 0.0;
-        }
-#pragma unroll
-        for (int j = 0; j < kKeygenItems; ++j) {
-            const long long k = base + j * 256 + threadIdx.x;
-            const bool ok = k < N;
-            const unsigned long long key = mex_key(x[j], y[j], z[j]);
-            if (ok) {
-                keys[k] = key;
-                idx[k] = (unsigned)k;
-                if (PACK) { pk[2 * k] = make_double2(x[j], y[j]); pk[2 * k + 1] = make_double2(z[j], mk[j]); }
-#pragma unroll
-                for (int p = 0; p < kSortPasses - 1; ++p) atomicAdd(&sh[p * 256 + (unsigned)((key >> (8 * p)) & 255u)], 1u);
-            }
-            const unsigned top = ok ? (unsigned)(key >> 56) : 0x100u;   // inactive lanes form their own group
-            const unsigned peers = __match_any_sync(0xffffffffu, top);
-            if (ok && (peers & ((1u << lane) - 1u)) == 0u) atomicAdd(&sh[(kSortPasses - 1) * 256 + top], (unsigned)__popc(peers));
-        }
-    }
-    __syncthreads();
-    for (int i = threadIdx.x; i < kSortPasses * 256; i += 256)
-        if (sh[i]) atomicAdd(&hist[i], sh[i]);
-}
-
-// =========================================================================================================
-// M2: one stable LSD radix pass (8 bits) with decoupled lookback.
-// status word: [63:56] tag (2*pass+1 = tile aggregate, 2*pass+2 = inclusive prefix, anything else = not yet),
-//              [55:0] count.  The buffer is zeroed once per sort; tags of earlier passes read as "not yet".
-// Ranking: the lanes of a warp that hold the same digit are found with eight ballots (one per digit bit) —
-// the MATCH.ANY instruction iterates over the distinct values of the warp and was the kernel's bottleneck
-// (profiles/r1b_summary.md).  Launched with programmatic stream serialisation: the prologue (ticket, clearing the
-// counters) overlaps the tail of the preceding pass; griddepcontrol.wait orders every read of its output, and those
-// reads are L2-coherent loads (ld.global.cg), never the non-coherent path a const __restrict__ pointer would allow —
-// the block was resident before the producer finished.  (Extending the same launch mode to the other MEX kernels,
-// which read their inputs through the non-coherent path, produced wrong results at N = 2049 and was dropped.)
-// =========================================================================================================
-constexpr unsigned long long kCountMask = (1ull << 56) - 1;
-
-// Phase timestamps of the radix pass for the development harness (compiled out of the library).
-#ifdef ETICS_SORT_TRACE
-__device__ unsigned long long g_sort_trace[1 << 16][8];
-#define ETICS_TRACE(slot)                                                                              \
-    do {                                                                                               \
-        if (threadIdx.x == 0) {                                                                        \
-            unsigned long long t_;                                                                     \
-            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                                     \
-            g_sort_trace[blockIdx.x & 0xffff][slot] = t_;                                              \
-        }                                                                                              \
-    } while (0)
-#else
-#define ETICS_TRACE(slot) do {} while (0)
-#endif
-
-template <int ITEMS>
-struct SortSmem {
-    uint2 warp_hist[kSortWarps][256];      // per warp and digit: .x = match mask of the item being ranked, .y = digit
-                                           // count so far -> exclusive offset of the warp's keys inside the tile
-    unsigned gbase[256];                   // global position of the tile's first key of digit d, minus local_off[d]
-    unsigned scan_tmp[kSortWarps];
-    unsigned tile;
-    unsigned long long keys[kSortThreads * ITEMS];
-    unsigned idx[kSortThreads * ITEMS];
-};
-
-__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
-
-__device__ __forceinline__ unsigned block_exclusive_scan_256(unsigned v, unsigned* tmp) {
-    // kSortThreads == 256 threads, one value each
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    unsigned inc = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += t;
-    }
-    if (lane == 31) tmp[warp] = inc;
-    __syncthreads();
-    unsigned woff = 0;
-#pragma unroll
-    for (int w = 0; w < kSortWarps; ++w) {
-        const unsigned t = tmp[w];
-        if (w < warp) woff += t;
-    }
-    __syncthreads();
-    return woff + inc - v;
-}
-
-// MINB = resident blocks per SM the register allocation is sized for.  A sort whose tiles all fit in one wave at two
-// blocks per SM (N ~ 10^6) runs faster with 123 registers and no spills (8 passes: 125 -> 117 us); a large sort wants the
-// third resident block (N = 10^8: 6.3 ms against 7.2 ms).
-template <int ITEMS, int MINB>
-__global__ void __launch_bounds__(kSortThreads, MINB)
-mex_radix_pass_kernel(const unsigned long long* __restrict__ keys_in, const unsigned* __restrict__ idx_in,
-                      unsigned long long* __restrict__ keys_out, unsigned* __restrict__ idx_out,
-                      long long N, int pass, const unsigned* __restrict__ hist, unsigned* __restrict__ tickets,
-                      unsigned long long* status) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    SortSmem<ITEMS>& S = *reinterpret_cast<SortSmem<ITEMS>*>(smem_raw);
-    constexpr int TILE = kSortThreads * ITEMS;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int shift = 8 * pass;
-
-    ETICS_TRACE(0);
-    pdl_launch_dependents();
-    if (tid == 0) S.tile = atomicAdd(&tickets[pass], 1u);   // tiles are numbered in the order they start running
-#pragma unroll
-    for (int w = 0; w < kSortWarps; ++w) S.warp_hist[w][tid] = make_uint2(0u, 0u);
-    __syncthreads();
-    const long long tile = S.tile;
-    const long long base = tile * TILE + (long long)warp * (32 * ITEMS);
-    pdl_wait();
-    ETICS_TRACE(1);
-
-    // ---- load (warp-striped: item i of the warp's slice sits at base + 32 i + lane) and rank ------------------
-    unsigned long long key[ITEMS];
-    unsigned short rank[ITEMS];
-#pragma unroll
-    for (int i = 0; i < ITEMS; ++i) {
-        const long long k = base + 32 * i + lane;
-        key[i] = (k < N) ? __ldcg(keys_in + k) : ~0ull;   // padding sorts last in every pass and is never written (position >= N)
-    }
-    const unsigned hcount = __ldcg(hist + pass * 256 + tid);
-    ETICS_TRACE(2);
-    const unsigned lane_bit = 1u << lane, lt_mask = lane_bit - 1u;
-    uint2* wh = S.warp_hist[warp];
-    // Lanes holding the same digit find each other with eight ballots, one per digit bit.  (Measured on B200, per
-    // SM sub-partition: VOTE 8 cycles; MATCH.ANY 8 cycles per distinct value in the warp, i.e. ~230 for random
-    // digits; a shared-memory atomicOr of lane bits ~1 lane per cycle per SM — both slower than 8 x VOTE.)
-#pragma unroll
-    for (int i = 0; i < ITEMS; ++i) {
-        const unsigned d = (unsigned)(key[i] >> shift) & 255u;
-        unsigned peers = 0xffffffffu;
-#pragma unroll
-        for (int b = 0; b < 8; ++b) {
-            const bool bit = (d >> b) & 1u;
-            const unsigned vote = __ballot_sync(0xffffffffu, bit);
-            peers &= bit ? vote : ~vote;
-        }
-        const unsigned lower = peers & lt_mask;
-        const unsigned prior = wh[d].y;            // every lane of the group reads the count before the leader advances it
-        rank[i] = (unsigned short)(prior + __popc(lower));
-        __syncwarp();
-        if (lower == 0u) wh[d].y = prior + __popc(peers);
-        __syncwarp();
-    }
-    ETICS_TRACE(3);
-    __syncthreads();
-
-    // ---- thread d owns digit d: warp offsets, tile count, lookback ---------------------------------------------
-    unsigned count = 0;
-#pragma unroll
-    for (int w = 0; w < kSortWarps; ++w) {
-        const unsigned t = S.warp_hist[w][tid].y;
-        S.warp_hist[w][tid].y = count;
-        count += t;
-    }
-    const unsigned long long tag_agg = (unsigned long long)(2 * pass + 1) << 56;
-    const unsigned long long tag_inc = (unsigned long long)(2 * pass + 2) << 56;
-    volatile unsigned long long* my_status = status + (size_t)tile * 256 + tid;
-    if (tile > 0) *my_status = tag_agg | count;
-
-    const unsigned loc = block_exclusive_scan_256(count, S.scan_tmp);
-#pragma unroll
-    for (int w = 0; w < kSortWarps; ++w) S.warp_hist[w][tid].y += loc;   // -> position inside the tile
-    __syncthreads();
-
-    // ---- reorder inside the tile (stable); keys, ranks and payload leave the registers before the look-back ------
-    {
-        unsigned pay[ITEMS];
-#pragma unroll
-        for (int i = 0; i < ITEMS; ++i) {
-            const long long k = base + 32 * i + lane;
-            pay[i] = (k < N) ? __ldcg(idx_in + k) : 0u;
-        }
-#pragma unroll
-        for (int i = 0; i < ITEMS; ++i) {
-            const unsigned d = (unsigned)(key[i] >> shift) & 255u;
-            const unsigned p = wh[d].y + rank[i];
-            S.keys[p] = key[i];
-            S.idx[p] = pay[i];
-        }
-    }
-    const unsigned hbase = block_exclusive_scan_256(hcount, S.scan_tmp);   // global start of bucket d
-
-    ETICS_TRACE(4);
-    // look back kLookW tiles at a time (independent loads in flight), consume them nearest first
-    unsigned long long excl = 0;
-    if (tile > 0) {
-        long long t = tile - 1;
-        bool done = false;
-        while (!done) {
-            unsigned long long v[kLookW];
-#pragma unroll
-            for (int j = 0; j < kLookW; ++j)
-                v[j] = (t - j >= 0) ? *(volatile unsigned long long*)(status + (size_t)(t - j) * 256 + tid) : tag_inc;
-            int used = kLookW;
-#pragma unroll
-            for (int j = 0; j < kLookW; ++j) {
-                if (!done && used == kLookW) {
-                    const unsigned long long tag = v[j] & ~kCountMask;
-                    if (tag == tag_inc) { excl += v[j] & kCountMask; done = true; }
-                    else if (tag == tag_agg) excl += v[j] & kCountMask;
-                    else used = j;   // not posted yet: poll again from this tile
-                }
-            }
-            t -= used;
-            if (used == 0) __nanosleep(40);
-        }
-    }
-    ETICS_TRACE(5);
-    *my_status = tag_inc | (excl + count);
-    S.gbase[tid] = hbase + (unsigned)excl - loc;
-    __syncthreads();
-
-    // ---- write runs of equal digits -------------------------------------------------------------------------------
-    ETICS_TRACE(6);
-#pragma unroll
-    for (int i = 0; i < ITEMS; ++i) {
-        const unsigned j = i * kSortThreads + tid;
-        const unsigned long long kk = S.keys[j];
-        const unsigned d = (unsigned)(kk >> shift) & 255u;
-        const unsigned g = S.gbase[d] + j;
-        if ((long long)g < N) { keys_out[g] = kk; idx_out[g] = S.idx[j]; }
-    }
-    ETICS_TRACE(7);
-}
 
 // =========================================================================================================
 // M3: gather into geometry records.  Record of the particle at sorted position p = tile*TP + c*K + k
@@ -868,77 +575,10 @@ mex_unpack_kernel(const double2* __restrict__ out4, long long N, double* __restr
 // Host side.
 // ---------------------------------------------------------------------------------------------------------
 #if ETICS_MEX_PART == 0
-template <int ITEMS, int MINB>
-static cudaError_t radix_passes_enqueue(unsigned long long* const* kbuf, unsigned* const* ibuf, unsigned long long* keys_out,
-                                        unsigned* idx_out, long long N, const unsigned* hist, unsigned* tickets,
-                                        unsigned long long* status, cudaStream_t st) {
-    auto kern = mex_radix_pass_kernel<ITEMS, MINB>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem<ITEMS>));
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
-    constexpr int TILE = kSortThreads * ITEMS;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)((N + TILE - 1) / TILE));
-    cfg.blockDim = dim3(kSortThreads);
-    cfg.dynamicSmemBytes = sizeof(SortSmem<ITEMS>);
-    cfg.stream = st;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    for (int pass = 0; pass < kSortPasses; ++pass) {
-        const bool last = pass == kSortPasses - 1;
-        cudaError_t e = cudaLaunchKernelEx(&cfg, kern, (const unsigned long long*)kbuf[pass & 1], (const unsigned*)ibuf[pass & 1],
-                                           last ? keys_out : kbuf[(pass + 1) & 1], last ? idx_out : ibuf[(pass + 1) & 1],
-                                           N, pass, hist, tickets, status);
-        if (e != cudaSuccess) return e;
-    }
-    return cudaSuccess;
-}
-
-// pk == nullptr: sort only (no packed particle records)
-static cudaError_t mex_sort_enqueue(const double* pos, const double* mass, long long N, const MexLayout& L, char* ws,
-                                    unsigned long long* keys_out, unsigned* idx_out, bool pack, cudaStream_t st,
-                                    cudaEvent_t ev_keygen = nullptr) {
-    unsigned* hist = reinterpret_cast<unsigned*>(ws + L.off_hist);
-    unsigned* tickets = reinterpret_cast<unsigned*>(ws + L.off_ticket);
-    unsigned long long* status = reinterpret_cast<unsigned long long*>(ws + L.off_status);
-    unsigned long long* kbuf[2] = {reinterpret_cast<unsigned long long*>(ws + L.off_keysA),
-                                   reinterpret_cast<unsigned long long*>(ws + L.off_keysB)};
-    unsigned* ibuf[2] = {reinterpret_cast<unsigned*>(ws + L.off_idxA), reinterpret_cast<unsigned*>(ws + L.off_idxB)};
-    double2* pk = reinterpret_cast<double2*>(ws + L.off_pk);
-
-    cudaError_t e = cudaMemsetAsync(ws + L.off_zero, 0, L.zero_bytes, st);
-    if (e != cudaSuccess) return e;
-    const long long per_block = 256 * kKeygenItems;
-    long long kg_blocks = (N + per_block - 1) / per_block;
-    if (kg_blocks > 148 * 8) kg_blocks = 148 * 8;
-    if (pack) mex_keygen_kernel<true><<<(unsigned)kg_blocks, 256, 0, st>>>(pos, mass, N, kbuf[0], ibuf[0], hist, pk);
-    else mex_keygen_kernel<false><<<(unsigned)kg_blocks, 256, 0, st>>>(pos, nullptr, N, kbuf[0], ibuf[0], hist, nullptr);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    if (ev_keygen) cudaEventRecord(ev_keygen, st);
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 148;
-    }
-    const long long tiles16 = (N + kSortThreads * 16 - 1) / (kSortThreads * 16);
-    if (N < kSortSmallN) e = radix_passes_enqueue<8, 4>(kbuf, ibuf, keys_out, idx_out, N, hist, tickets, status, st);
-    else if (tiles16 <= 2ll * sms) e = radix_passes_enqueue<16, 2>(kbuf, ibuf, keys_out, idx_out, N, hist, tickets, status, st);
-    else e = radix_passes_enqueue<16, 3>(kbuf, ibuf, keys_out, idx_out, N, hist, tickets, status, st);
-    if (e != cudaSuccess) return e;
-    return cudaSuccess;
-}
-
 cudaError_t mex_sort_launch(const double* pos, long long N, unsigned long long* keys_sorted, unsigned int* perm,
                             void* ws, cudaStream_t st) {
     const MexLayout L = make_mex_layout(N, 0);
-    return mex_sort_enqueue(pos, nullptr, N, L, static_cast<char*>(ws), keys_sorted, perm, false, st);
+    return mex_sort_enqueue(pos, nullptr, N, L, static_cast<char*>(ws), perm, keys_sorted, false, st, nullptr);
 }
 
 #endif   // ETICS_MEX_PART == 0
@@ -1016,10 +656,9 @@ static cudaError_t mex_force_enqueue(const double* pos, const double* mass, long
                                      double* acc, double* pot, void* wsv, cudaStream_t st, cudaEvent_t* ev) {
     const MexLayout L = make_mex_layout(N, lmax);
     char* ws = static_cast<char*>(wsv);
-    unsigned long long* keysA = reinterpret_cast<unsigned long long*>(ws + L.off_keysA);
-    unsigned* idxA = reinterpret_cast<unsigned*>(ws + L.off_idxA);
+    unsigned* idxA = reinterpret_cast<unsigned*>(ws + L.off_perm);
     if (ev) cudaEventRecord(ev[0], st);
-    cudaError_t e = mex_sort_enqueue(pos, mass, N, L, ws, keysA, idxA, true, st, ev ? ev[1] : nullptr);   // pass 7: buffer B -> A
+    cudaError_t e = mex_sort_enqueue(pos, mass, N, L, ws, idxA, nullptr, true, st, ev ? ev[1] : nullptr);
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[2], st);
     const long long gthreads = L.tiles * kMexTile;

@@ -1,0 +1,59 @@
+// mex_common.cuh — workspace layout and launch plumbing shared by the MEX translation units (mex_sort.cu: M1–M2,
+// mex.cu: M3–M7).  Never included by oracle/.
+#pragma once
+
+#include "etics_common.cuh"
+
+namespace etics {
+
+// ---- sort geometry (mex_sort.cu) ---------------------------------------------------------------------------
+constexpr int kSortThreads = 256;
+constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kSortDigitBits = 11;                 // widest digit of a pass
+constexpr int kSortBins = 1 << kSortDigitBits;     // 2048
+constexpr int kSortMaxPasses = 3;
+constexpr int kSortPrefixBits = kSortDigitBits * kSortMaxPasses;   // 33 key bits are radix-sorted, the rest is fixed up
+constexpr int kSortMinTile = kSortThreads * 16;    // the look-back status buffer is sized for the smallest tile
+
+// Header of the sort, in the zeroed part of the workspace.
+struct SortHeader {
+    unsigned long long inv_kmin;   // max over ~key (so that zero-initialisation works); kmin = ~inv_kmin
+    unsigned long long kmax;
+    unsigned tickets[4];           // one per pass: tiles are numbered in the order they start running
+    unsigned fallback;             // set by the fix-up when a run of equal prefixes is too long to fix locally
+    unsigned pad[3];
+};
+
+// ---- scan geometry (mex.cu) --------------------------------------------------------------------------------
+constexpr int kMexThreads = 32;          // a scan tile is one warp: lane = chunk of kMexK consecutive sorted particles
+constexpr int kMexK = 8;
+constexpr int kMexTile = kMexThreads * kMexK;
+constexpr int kRecFields = 8;            // r, 1/r, cos th, sin th, cos ph, sin ph, mass, (spare)
+
+struct MexLayout {
+    long long N;
+    int lmax;
+    long long sort_rows;        // look-back status rows (one per smallest sort tile)
+    long long tiles, chunks;    // scan tiles; chunks = tiles * kMexThreads
+    int rows;                   // running sums per particle: 2 directions x (cos,sin) x (l,m)
+    size_t off_zero, zero_bytes;   // [SortHeader | hist passes x kSortBins u32 | status passes x sort_rows x kSortBins u32]
+    size_t off_hdr, off_hist, off_status;
+    size_t off_keys;            // fp64 bit patterns of r^2 by original index (8N)
+    size_t off_wordsA, off_wordsB;   // packed (key prefix | index) words (8N each)
+    size_t off_perm;            // sorted order: perm[rank] = original index (4N)
+    size_t off_itmp;            // second index buffer of the fallback sort (4N)
+    size_t off_pk;              // (x, y, z, m) by original index, one 32-byte sector per particle; later the (Phi, a) records
+    size_t off_rec, off_idxT, off_pre, off_tot;
+    size_t total;
+};
+
+MexLayout make_mex_layout(long long N, int lmax);   // mex.cu part 0
+
+// mex_sort.cu: M1–M2.  perm_out[rank] = original index; keys_sorted_out may be null; pack: also write the (x,y,z,m)
+// records at L.off_pk.  ev_keygen (optional) is recorded after the key generation.
+cudaError_t mex_sort_enqueue(const double* pos, const double* mass, long long N, const MexLayout& L, char* ws,
+                             unsigned* perm_out, unsigned long long* keys_sorted_out, bool pack, cudaStream_t st,
+                             cudaEvent_t ev_keygen);
+cudaError_t mex_sort_init_device();
+
+}  // namespace etics

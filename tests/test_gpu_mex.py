@@ -85,6 +85,47 @@ def test_sort_all_equal_and_extreme_keys(E):
     check_sort(E, pos)
 
 
+def _wide_range_with_clusters(sizes, jitter, seed):
+    """Particles on the x axis: isolated ones spanning 40 octaves of r^2 (so that the sort drops the low key bits) plus
+    clusters whose members differ only in those low bits (relative spacing `jitter`)."""
+    rng = np.random.default_rng(seed)
+    x = [10.0 ** rng.uniform(-3.0, 3.0, 4000)]
+    for n in sizes:
+        x0 = 10.0 ** rng.uniform(-2.0, 2.0)
+        x.append(x0 * (1.0 + jitter * rng.permutation(n)))
+    x = np.concatenate(x)
+    pos = np.zeros((3, len(x)))
+    pos[0] = x[rng.permutation(len(x))]
+    return pos
+
+
+def test_sort_prefix_collisions_short_runs(E):
+    """Runs of 2..32 particles whose keys agree in the 33 sorted bits and differ below: the fix-up orders them."""
+    rng = np.random.default_rng(5)
+    pos = _wide_range_with_clusters(rng.integers(2, 33, 1500), 3e-13, seed=6)
+    keys0, _ = oracle.mex_sort(pos)
+    assert np.sum((keys0[1:] >> np.uint64(30)) == (keys0[:-1] >> np.uint64(30))) > 10_000   # many colliding neighbours
+    check_sort(E, pos)
+
+
+def test_sort_prefix_collisions_long_runs_fallback(E):
+    """Runs longer than the fix-up handles (two thin shells of thousands of particles, and 100 exact copies of one
+    particle) take the fallback sort; the result is the same bit-exact permutation."""
+    pos = _wide_range_with_clusters([5000, 3000, 33], 1e-14, seed=7)
+    check_sort(E, pos)
+    pos = _wide_range_with_clusters([2], 1e-14, seed=8)
+    pos = np.ascontiguousarray(np.concatenate([pos, np.repeat(pos[:, 17:18], 100, axis=1)], axis=1))
+    check_sort(E, pos)
+
+
+def test_sort_narrow_range_is_exact_without_fixup(E):
+    """A thin shell: the whole key range fits the sorted prefix (shift = 0), whatever N."""
+    rng = np.random.default_rng(11)
+    v = rng.normal(size=(3, 30_000))
+    pos = np.ascontiguousarray(v / np.sqrt(np.sum(v ** 2, axis=0)) * 1.25)
+    check_sort(E, pos)
+
+
 def test_sort_already_sorted_and_reversed(E):
     pos, _ = W.particles("hernquist", 20_000, seed=9)
     order = np.argsort(np.sum(pos ** 2, axis=0), kind="stable")
