@@ -22,7 +22,7 @@ SOURCES = [("etics_api.cu", "etics_api", []), ("scf.cu", "scf", []), ("probe.cu"
           [("mex.cu", f"mex_p{k}", [f"-DETICS_MEX_PART={k}"]) for k in range(4)]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-         "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+         "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("ETICS_NVCC_EXTRA", "").split()
 
 
 def _deps_mtime() -> float:

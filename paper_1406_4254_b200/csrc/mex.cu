@@ -111,17 +111,14 @@ __host__ __device__ constexpr double mex_dfact(int m) {   // (2m-1)!!
 MexLayout make_mex_layout(long long N, int lmax) {
     MexLayout L{};
     L.N = N; L.lmax = lmax;
-    L.sort_rows = (N + kSortMinTile - 1) / kSortMinTile;
     L.tiles = (N + kMexTile - 1) / kMexTile;
     L.chunks = L.tiles * kMexThreads;
     L.rows = mex_total_rows(lmax);
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += round_up(bytes, 256); return at; };
-    L.off_zero = o;
     L.off_hdr = take(sizeof(SortHeader));
-    L.off_hist = take((size_t)kSortMaxPasses * kSortBins * sizeof(unsigned));
-    L.off_status = take((size_t)kSortMaxPasses * L.sort_rows * kSortBins * sizeof(unsigned));
-    L.zero_bytes = o - L.off_zero;
+    L.off_seghist = take((size_t)kSortMaxSegs * kSortBins * sizeof(unsigned));
+    L.off_bintot = take((size_t)kSortBins * sizeof(unsigned));
     L.off_keys = take((size_t)N * 8);
     L.off_wordsA = take((size_t)N * 8);
     L.off_wordsB = take((size_t)N * 8);

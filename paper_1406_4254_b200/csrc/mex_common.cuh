@@ -13,15 +13,19 @@ constexpr int kSortDigitBits = 11;                 // widest digit of a pass
 constexpr int kSortBins = 1 << kSortDigitBits;     // 2048
 constexpr int kSortMaxPasses = 3;
 constexpr int kSortPrefixBits = kSortDigitBits * kSortMaxPasses;   // 33 key bits are radix-sorted, the rest is fixed up
-constexpr int kSortMinTile = kSortThreads * 16;    // the look-back status buffer is sized for the smallest tile
+constexpr int kSortMinTile = kSortThreads * 16;    // words per sort tile
+constexpr int kSortMaxSegs = 1024;                 // blocks of the persistent sort kernel (segment histogram rows)
 
 // Header of the sort, in the zeroed part of the workspace.
 struct SortHeader {
     unsigned long long inv_kmin;   // max over ~key (so that zero-initialisation works); kmin = ~inv_kmin
     unsigned long long kmax;
-    unsigned tickets[4];           // one per pass: tiles are numbered in the order they start running
     unsigned fallback;             // set by the fix-up when a run of equal prefixes is too long to fix locally
-    unsigned pad[3];
+    unsigned nheads;               // runs of equal prefixes listed by the fix-up
+    unsigned pad[10];
+#ifdef ETICS_SORT_PROF
+    unsigned long long prof[32];   // development: %globaltimer of block 0 at the phase boundaries
+#endif
 };
 
 // ---- scan geometry (mex.cu) --------------------------------------------------------------------------------
@@ -33,11 +37,11 @@ constexpr int kRecFields = 8;            // r, 1/r, cos th, sin th, cos ph, sin 
 struct MexLayout {
     long long N;
     int lmax;
-    long long sort_rows;        // look-back status rows (one per smallest sort tile)
     long long tiles, chunks;    // scan tiles; chunks = tiles * kMexThreads
     int rows;                   // running sums per particle: 2 directions x (cos,sin) x (l,m)
-    size_t off_zero, zero_bytes;   // [SortHeader | hist passes x kSortBins u32 | status passes x sort_rows x kSortBins u32]
-    size_t off_hdr, off_hist, off_status;
+    size_t off_hdr;             // SortHeader (zeroed by every call)
+    size_t off_seghist;         // digit histogram of every sort segment, kSortMaxSegs x kSortBins u32
+    size_t off_bintot;          // digit totals, kSortBins u32
     size_t off_keys;            // fp64 bit patterns of r^2 by original index (8N)
     size_t off_wordsA, off_wordsB;   // packed (key prefix | index) words (8N each)
     size_t off_perm;            // sorted order: perm[rank] = original index (4N)

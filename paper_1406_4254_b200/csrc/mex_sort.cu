@@ -3,27 +3,27 @@
 // sm_100a, no CUB/Thrust.
 //
 // The paper sorts whole particle structs with Thrust's merge sort.  Here the sort moves ONE 64-bit
-// word per particle and makes at most three passes:
+// word per particle, word_k = (prefix_k << ibits) | k with prefix_k = (key_k - kmin) >> shift: the leading B bits of the
+// key's offset from the smallest key above the ibits = bits(N-1) bits of the particle index.  The words go through
+// stable LSD passes over digits of the prefix (the index bits ride along); particles whose prefixes collide (the
+// key bits below `shift` were not sorted) form short runs that a fix-up orders by (full key, index).
 //
-//   mex_keygen_kernel   key_k = bits(r_k^2), rounding pinned (t = x*x; t = fma(y,y,t); t = fma(z,z,t)); the
-//                       (x,y,z,m) record of the particle as one 32-byte sector; min and max key of the set.
-//   mex_pack_kernel     word_k = (prefix_k << ibits) | k, prefix_k = (key_k - kmin) >> shift: the leading
-//                       B = min(33, bits(kmax - kmin)) bits of the key's offset from the smallest key, above the
-//                       ibits = bits(N-1) bits of the particle index; digit histograms of all passes.
-//   mex_radix_pass_kernel  one stable LSD pass over a digit of <= 11 bits of the prefix ("onesweep": ranks inside
-//                       the tile, decoupled look-back over the preceding tiles' digit counts — integers, so the
-//                       result does not depend on timing — one coalesced write).  The index bits ride along.
-//   mex_fixup_kernel    particles whose prefixes collide (the key bits below `shift` were not sorted) form short runs;
-//                       the thread at the head of a run orders it by (full key, index).  For smooth particle
-//                       distributions a fraction ~N / 2^27 per octave of r^2 collides.  shift = 0: nothing to do.
-//   mex_sort_fallback_kernel   a run longer than kFixMaxRun (many particles within 2^shift ulps of each other, yet
-//                       not all equal: e.g. two thin shells) raises a flag and this plain single-block LSD sort
-//                       of the full keys redoes the job — correct for any input, slow, never taken by the paper's workloads.
-//
-// Why 33 bits: an r^2 range of 44 octaves (r from 1e-4 to 300) needs 6 exponent bits, which leaves 27 mantissa bits
-// in the prefix; three 11-bit passes over 8-byte words move 48 bytes per particle where eight 8-bit passes over
-// (key, index) pairs moved 192.
+// Every pass is histogram -> scan -> scatter over SEGMENTS (consecutive tiles owned by one block): no block ever
+// waits for another block's progress, and everything is integer work in a fixed order.
+//   N <= one tile per resident block (~1.2e6): ONE cooperative kernel, grid-wide barriers between the phases, B = 33,
+//     three 11-bit passes (the sort is a single wave and latency-bound: fewer, wider passes).
+//   larger N: one kernel per phase, B = 36, four 9-bit passes (bandwidth-bound: with 2048 digit values a 4096-word tile
+//     scatters runs of two words; 512 values give 64-byte runs).
+//   mex_sort_fallback_kernel: a run longer than kFixMaxRun (many particles within 2^shift ulps of each other, yet not
+//     all equal: e.g. two thin shells) raises a flag and this plain single-block LSD sort of the full keys redoes the
+//     job — correct for any input, slow, never taken by the paper's workloads.
+#include <cooperative_groups.h>
+
+#include <cstdlib>
+
 #include "mex_common.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace etics {
 
@@ -47,20 +47,21 @@ __host__ __device__ inline int bit_length64(unsigned long long v) {
     return n;
 }
 
-__host__ __device__ inline SortPlan make_sort_plan(unsigned long long kmin, unsigned long long kmax, long long N) {
+__host__ __device__ inline SortPlan make_sort_plan(unsigned long long kmin, unsigned long long kmax, long long N,
+                                                   int prefix_bits, int digit_bits) {
     SortPlan p;
     p.kmin = kmin;
     p.ibits = bit_length64((unsigned long long)(N - 1));
     const int nbits = bit_length64(kmax - kmin);
-    p.B = nbits < kSortPrefixBits ? nbits : kSortPrefixBits;
+    p.B = nbits < prefix_bits ? nbits : prefix_bits;
     p.shift = nbits - p.B;
-    p.passes = (p.B + kSortDigitBits - 1) / kSortDigitBits;
+    p.passes = (p.B + digit_bits - 1) / digit_bits;
     return p;
 }
 
-__device__ __forceinline__ SortPlan load_plan(const SortHeader* hdr, long long N) {
+__device__ __forceinline__ SortPlan load_plan(const SortHeader* hdr, long long N, int prefix_bits, int digit_bits) {
     const unsigned long long inv = __ldcg(&hdr->inv_kmin), kmax = __ldcg(&hdr->kmax);
-    return make_sort_plan(~inv, kmax, N);
+    return make_sort_plan(~inv, kmax, N, prefix_bits, digit_bits);
 }
 
 // =========================================================================================================
@@ -73,129 +74,105 @@ __device__ __forceinline__ unsigned long long mex_key(double x, double y, double
     return (unsigned long long)__double_as_longlong(t);   // r^2 >= 0: the bit pattern is monotone in r^2
 }
 
-constexpr int kKeygenItems = 4;
-
-// PACK: also write (x, y, z, m) of particle k as one 32-byte record pk[k], so that the gather after the sort reads
-// one aligned sector per particle instead of four.
-template <bool PACK>
-__global__ void __launch_bounds__(256)
-mex_keygen_kernel(const double* __restrict__ pos, const double* __restrict__ mass, long long N,
-                  unsigned long long* __restrict__ keys, double2* __restrict__ pk, SortHeader* __restrict__ hdr) {
-    __shared__ unsigned long long s_inv[8], s_max[8];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    unsigned long long inv = 0, mx = 0;
-    const long long stride = (long long)gridDim.x * 256 * kKeygenItems;
-    for (long long base = (long long)blockIdx.x * 256 * kKeygenItems; base < N; base += stride) {
-        double x[kKeygenItems], y[kKeygenItems], z[kKeygenItems], mk[kKeygenItems];
-#pragma unroll
-        for (int j = 0; j < kKeygenItems; ++j) {
-            const long long k = base + j * 256 + threadIdx.x;
-            const bool ok = k < N;
-            x[j] = ok ? pos[k] : 0.0; y[j] = ok ? pos[N + k] : 0.0; z[j] = ok ? pos[2 * N + k] : 0.0;
-            if (PACK) mk[j] = ok ? mass[k] : 0.0;
-        }
-#pragma unroll
-        for (int j = 0; j < kKeygenItems; ++j) {
-            const long long k = base + j * 256 + threadIdx.x;
-            if (k < N) {
-                const unsigned long long key = mex_key(x[j], y[j], z[j]);
-                keys[k] = key;
-                if (PACK) { pk[2 * k] = make_double2(x[j], y[j]); pk[2 * k + 1] = make_double2(z[j], mk[j]); }
-                inv = max(inv, ~key);
-                mx = max(mx, key);
-            }
-        }
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        inv = max(inv, __shfl_xor_sync(0xffffffffu, inv, o));
-        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-    }
-    if (lane == 0) { s_inv[warp] = inv; s_max[warp] = mx; }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-#pragma unroll
-        for (int w = 1; w < 8; ++w) { inv = max(inv, s_inv[w]); mx = max(mx, s_max[w]); }
-        atomicMax(&hdr->inv_kmin, inv);   // integer atomics: the result does not depend on their order
-        atomicMax(&hdr->kmax, mx);
-    }
-}
-
 // =========================================================================================================
-// Packed words and the digit histograms of every pass.
-// =========================================================================================================
-__global__ void __launch_bounds__(256)
-mex_pack_kernel(const unsigned long long* __restrict__ keys, long long N, const SortHeader* __restrict__ hdr,
-                unsigned long long* __restrict__ words, unsigned* __restrict__ hist) {
-    __shared__ unsigned sh[kSortMaxPasses * kSortBins];
-    const SortPlan pl = load_plan(hdr, N);
-    for (int i = threadIdx.x; i < kSortMaxPasses * kSortBins; i += 256) sh[i] = 0;
-    __syncthreads();
-    const long long stride = (long long)gridDim.x * 256 * kKeygenItems;
-    for (long long base = (long long)blockIdx.x * 256 * kKeygenItems; base < N; base += stride) {
-        unsigned long long key[kKeygenItems];
-#pragma unroll
-        for (int j = 0; j < kKeygenItems; ++j) {
-            const long long k = base + j * 256 + threadIdx.x;
-            key[j] = (k < N) ? keys[k] : 0ull;
-        }
-#pragma unroll
-        for (int j = 0; j < kKeygenItems; ++j) {
-            const long long k = base + j * 256 + threadIdx.x;
-            if (k < N) {
-                const unsigned long long pre = (key[j] - pl.kmin) >> pl.shift;
-                words[k] = (pre << pl.ibits) | (unsigned long long)k;
-#pragma unroll
-                for (int p = 0; p < kSortMaxPasses; ++p)
-                    if (p < pl.passes) atomicAdd(&sh[p * kSortBins + (unsigned)((pre >> pl.lo(p)) & ((1u << pl.w(p)) - 1u))], 1u);
-            }
-        }
-    }
-    __syncthreads();
-    for (int i = threadIdx.x; i < kSortMaxPasses * kSortBins; i += 256)
-        if (sh[i]) atomicAdd(&hist[i], sh[i]);
-}
-
-// =========================================================================================================
-// M2: one stable LSD radix pass with decoupled look-back.
+// M1–M2 in ONE persistent cooperative kernel (grid = every block the GPU holds at once; grid-wide barriers
+// between the phases, no polling on other blocks' progress anywhere):
 //
-// Tile = 256 threads x ITEMS words, loaded warp-striped (item i of warp w at tile base + w*32*ITEMS + 32 i + lane), so the
-// order (warp, item, lane) is the order of the input.
-// Ranking: per warp and digit a 16-bit counter [tag:5 | count:11].  For every item the lanes stamp their lane
-// number on their digit's counter and read it back: if every lane finds its own stamp, all 32 digits of the item
-// are distinct (78 % of the items for uniformly distributed 11-bit digits) and the rank is simply the counter;
-// otherwise the lanes that share a digit find each other with one ballot per digit bit.  (Measured in round 1:
-// MATCH.ANY iterates over the distinct values of a warp, ~230 cycles for random digits; shared-memory atomics do
-// not return ranks in lane order.)
-// Status word of (tile, digit): bit 31 = inclusive prefix (31-bit count), else bit 30 = tile aggregate, else not yet
-// posted.  One status array per pass, zeroed with the header.
-// Launched with programmatic stream serialisation: the prologue (ticket, clearing the counters) overlaps the tail
-// of the preceding kernel; griddepcontrol.wait orders every read of its output, and those reads are L2-coherent.
+//   phase K   keys, (x,y,z,m) records, min / max key (integer atomics)
+//   phase W   packed words; digit histogram of pass 0 per SEGMENT (a segment = the consecutive tiles one block owns)
+//   per pass: phase S   exclusive scan of the segment histograms along the segments, one warp per digit value
+//             phase P   every block walks its tiles in order: rank inside the tile (stable), positions from the
+//                       segment's scanned offsets plus a running count per digit, one coalesced write
+//             phase H   segment histograms of the next pass's digit
+//   phase F   fix-up of colliding prefixes -> permutation (and sorted keys)
+//
+// Everything is integer work in a fixed order, so the result is unique.  Data written by one block and read by
+// another after a barrier is read with ld.global.cg (L2), never through the non-coherent path.
 // =========================================================================================================
-constexpr unsigned kFlagIncl = 0x80000000u, kFlagAgg = 0x40000000u;
-constexpr int kBinsPerThread = kSortBins / kSortThreads;   // 8: thread t owns digits 8t..8t+7 in the offset phases
-constexpr int kLookW = 2;                                  // status rows in flight per look-back round
-static_assert(kBinsPerThread == 8, "the offset phases move the eight 16-bit counters of a thread as one 16-byte vector");
-
-template <int ITEMS>
-struct SortSmem {
-    unsigned short cnt[kSortWarps][kSortBins];   // ranking: [tag | count]; afterwards position of (warp, digit) inside the tile
-    unsigned gbase[kSortBins];                   // global position of the tile's first word of digit d, minus its tile position
-    unsigned scan_tmp[kSortWarps];
-    unsigned tile;
-    unsigned long long stage[kSortThreads * ITEMS];
+struct SortParams {
+    const double* pos;
+    const double* mass;
+    long long N;
+    unsigned long long* keys;
+    double2* pk;              // null: no records
+    SortHeader* hdr;
+    unsigned long long* bufA;
+    unsigned long long* bufB;
+    unsigned* seg_hist;       // [nseg][kSortBins]
+    unsigned* bin_tot;        // [kSortBins]
+    unsigned* perm;
+    unsigned long long* keys_sorted;   // may be null
+    long long tiles, tps;     // tiles of kSortTile words; tiles per segment
+    int nseg;
+    int prefix_bits, digit_bits;   // key bits that are radix-sorted; width of a digit (<= kSortDigitBits)
 };
 
-__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+constexpr int kSortItems = 16;
+constexpr int kSortTile = kSortThreads * kSortItems;       // 4096 words
+static_assert(kSortTile == kSortMinTile, "workspace sizing");
+constexpr int kScanStrip = 8;                              // digit values per strip of the segment scan (one 32-byte sector)
 
-__device__ __forceinline__ uint4 ld_volatile_v4(const unsigned* p) {
-    uint4 v;
-    asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
-    return v;
+// DB = bits of a digit (compile time: 11 for the single-wave sort, 9 for the bandwidth-bound one).
+template <int DB>
+struct SortSmem {
+    static constexpr int BINS = 1 << DB;
+    static constexpr int BPT = BINS / kSortThreads;   // thread t owns digits BPT t .. BPT t + BPT - 1 in the offset steps
+    static_assert(BPT >= 2 && BPT % 2 == 0 && DB <= kSortDigitBits, "16-bit counters are moved in 32-bit pairs");
+    unsigned short cnt[kSortWarps][BINS];   // ranking: [tag | count]; afterwards position of (warp, digit) inside the tile
+    unsigned gbase[BINS];                   // global position of the tile's first word of digit d, minus its tile position
+    unsigned run[BINS];                     // scatter: next free global position of digit d for this segment; histogram phases: counts
+    unsigned scan_tmp[kSortWarps];
+    unsigned long long red[2][kSortWarps];
+    unsigned long long stage[kSortTile];    // scatter: the tile in output order; scan: a strip of the segment histograms
+};
+
+template <int W>
+__device__ __forceinline__ void ld_words(const unsigned* p, unsigned (&v)[W]) {
+    if constexpr (W % 4 == 0) {
+#pragma unroll
+        for (int i = 0; i < W / 4; ++i) {
+            const uint4 t = reinterpret_cast<const uint4*>(p)[i];
+            v[4 * i] = t.x; v[4 * i + 1] = t.y; v[4 * i + 2] = t.z; v[4 * i + 3] = t.w;
+        }
+    } else if constexpr (W % 2 == 0) {
+#pragma unroll
+        for (int i = 0; i < W / 2; ++i) {
+            const uint2 t = reinterpret_cast<const uint2*>(p)[i];
+            v[2 * i] = t.x; v[2 * i + 1] = t.y;
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < W; ++i) v[i] = p[i];
+    }
 }
-__device__ __forceinline__ void st_volatile_v4(unsigned* p, uint4 v) {
-    asm volatile("st.volatile.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+template <int W>
+__device__ __forceinline__ void st_words(unsigned* p, const unsigned (&v)[W]) {
+    if constexpr (W % 4 == 0) {
+#pragma unroll
+        for (int i = 0; i < W / 4; ++i) reinterpret_cast<uint4*>(p)[i] = make_uint4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+    } else if constexpr (W % 2 == 0) {
+#pragma unroll
+        for (int i = 0; i < W / 2; ++i) reinterpret_cast<uint2*>(p)[i] = make_uint2(v[2 * i], v[2 * i + 1]);
+    } else {
+#pragma unroll
+        for (int i = 0; i < W; ++i) p[i] = v[i];
+    }
+}
+template <int W>
+__device__ __forceinline__ void ldcg_words(const unsigned* p, unsigned (&v)[W]) {
+    if constexpr (W % 4 == 0) {
+#pragma unroll
+        for (int i = 0; i < W / 4; ++i) {
+            const uint4 t = __ldcg(reinterpret_cast<const uint4*>(p) + i);
+            v[4 * i] = t.x; v[4 * i + 1] = t.y; v[4 * i + 2] = t.z; v[4 * i + 3] = t.w;
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < W / 2; ++i) {
+            const uint2 t = __ldcg(reinterpret_cast<const uint2*>(p) + i);
+            v[2 * i] = t.x; v[2 * i + 1] = t.y;
+        }
+    }
 }
 
 __device__ __forceinline__ unsigned block_exclusive_scan_256(unsigned v, unsigned* tmp) {
@@ -219,239 +196,338 @@ __device__ __forceinline__ unsigned block_exclusive_scan_256(unsigned v, unsigne
     return woff + inc - v;
 }
 
-template <int ITEMS, int MINB>
-__global__ void __launch_bounds__(kSortThreads, MINB)
-mex_radix_pass_kernel(const unsigned long long* __restrict__ bufA, unsigned long long* __restrict__ bufB,
-                      long long N, int pass, SortHeader* __restrict__ hdr, const unsigned* __restrict__ hist,
-                      unsigned* status_all, long long status_rows) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    SortSmem<ITEMS>& S = *reinterpret_cast<SortSmem<ITEMS>*>(smem_raw);
-    constexpr int TILE = kSortThreads * ITEMS;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+constexpr int kKeygenItems = 4;
 
-    pdl_launch_dependents();
-    if (tid == 0) S.tile = atomicAdd(&hdr->tickets[pass], 1u);   // tiles are numbered in the order they start running
-    {
-        uint4* c = reinterpret_cast<uint4*>(&S.cnt[0][0]);
-        constexpr int kVec = kSortWarps * kSortBins * 2 / 16;
+// phase K
+__device__ __forceinline__ void sort_phase_keys(const SortParams& P, unsigned long long (*red)[kSortWarps]) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const long long N = P.N;
+    unsigned long long inv = 0, mx = 0;
+    const long long stride = (long long)gridDim.x * kSortThreads * kKeygenItems;
+    for (long long base = (long long)blockIdx.x * kSortThreads * kKeygenItems; base < N; base += stride) {
+        double x[kKeygenItems], y[kKeygenItems], z[kKeygenItems], mk[kKeygenItems];
 #pragma unroll
-        for (int i = 0; i < kVec / kSortThreads; ++i) c[i * kSortThreads + tid] = make_uint4(0u, 0u, 0u, 0u);
-    }
-    __syncthreads();
-    const long long tile = S.tile;
-    pdl_wait();
-
-    const SortPlan pl = load_plan(hdr, N);
-    if (pass >= pl.passes) return;   // fewer digits than passes: the data stays where it is
-    const unsigned long long* __restrict__ in = (pass & 1) ? bufB : bufA;
-    unsigned long long* __restrict__ out = (pass & 1) ? const_cast<unsigned long long*>(bufA) : bufB;
-    const int dshift = pl.ibits + pl.lo(pass);
-    const unsigned dmask = (1u << pl.w(pass)) - 1u;
-    unsigned* status = status_all + (size_t)pass * status_rows * kSortBins;
-
-    // ---- load ---------------------------------------------------------------------------------------------
-    const long long base = tile * TILE + (long long)warp * (32 * ITEMS);
-    unsigned long long key[ITEMS];
+        for (int j = 0; j < kKeygenItems; ++j) {
+            const long long k = base + j * kSortThreads + threadIdx.x;
+            const bool ok = k < N;
+            x[j] = ok ? P.pos[k] : 0.0; y[j] = ok ? P.pos[N + k] : 0.0; z[j] = ok ? P.pos[2 * N + k] : 0.0;
+            mk[j] = (ok && P.pk) ? P.mass[k] : 0.0;
+        }
 #pragma unroll
-    for (int i = 0; i < ITEMS; ++i) {
-        const long long k = base + 32 * i + lane;
-        key[i] = (k < N) ? __ldcg(in + k) : ~0ull;   // padding sorts last in every pass and is never written (position >= N)
-    }
-    // global start of every bucket: exclusive scan of the pass's histogram
-    unsigned hb[kBinsPerThread];
-    {
-        const uint4 h0 = __ldcg(reinterpret_cast<const uint4*>(hist + pass * kSortBins + kBinsPerThread * tid));
-        const uint4 h1 = __ldcg(reinterpret_cast<const uint4*>(hist + pass * kSortBins + kBinsPerThread * tid) + 1);
-        hb[0] = h0.x; hb[1] = h0.y; hb[2] = h0.z; hb[3] = h0.w; hb[4] = h1.x; hb[5] = h1.y; hb[6] = h1.z; hb[7] = h1.w;
-        unsigned run = 0;
-#pragma unroll
-        for (int q = 0; q < kBinsPerThread; ++q) { const unsigned t = hb[q]; hb[q] = run; run += t; }
-        const unsigned off = block_exclusive_scan_256(run, S.scan_tmp);
-#pragma unroll
-        for (int q = 0; q < kBinsPerThread; ++q) hb[q] += off;
-    }
-
-    // ---- rank ---------------------------------------------------------------------------------------------
-    unsigned short rank[ITEMS];
-    volatile unsigned short* cw = S.cnt[warp];
-    const unsigned lt_mask = (1u << lane) - 1u;
-#pragma unroll
-    for (int i = 0; i < ITEMS; ++i) {
-        const unsigned d = (unsigned)(key[i] >> dshift) & dmask;
-        const unsigned c = cw[d] & 0x7ffu;
-        __syncwarp();
-        cw[d] = (unsigned short)((lane << 11) | c);
-        __syncwarp();
-        const bool own = (cw[d] >> 11) == (unsigned)lane;
-        if (__all_sync(0xffffffffu, own)) {
-            rank[i] = (unsigned short)c;
-            cw[d] = (unsigned short)(c + 1u);
-        } else {
-            unsigned peers = 0xffffffffu;
-#pragma unroll
-            for (int b = 0; b < kSortDigitBits; ++b) {
-                const bool bit = (d >> b) & 1u;
-                const unsigned vote = __ballot_sync(0xffffffffu, bit);
-                peers &= bit ? vote : ~vote;
+        for (int j = 0; j < kKeygenItems; ++j) {
+            const long long k = base + j * kSortThreads + threadIdx.x;
+            if (k < N) {
+                const unsigned long long key = mex_key(x[j], y[j], z[j]);
+                P.keys[k] = key;
+                if (P.pk) { P.pk[2 * k] = make_double2(x[j], y[j]); P.pk[2 * k + 1] = make_double2(z[j], mk[j]); }
+                inv = max(inv, ~key);
+                mx = max(mx, key);
             }
-            const unsigned lower = peers & lt_mask;
-            rank[i] = (unsigned short)(c + __popc(lower));
-            if (lower == 0u) cw[d] = (unsigned short)(c + __popc(peers));
         }
-        __syncwarp();
     }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        inv = max(inv, __shfl_xor_sync(0xffffffffu, inv, o));
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    }
+    if (lane == 0) { red[0][warp] = inv; red[1][warp] = mx; }
     __syncthreads();
-
-    // ---- thread t owns digits 8t..8t+7: per-warp counts -> exclusive over warps, tile totals -----------------
-    unsigned tot[kBinsPerThread];
-    {
-        uint4 run = make_uint4(0u, 0u, 0u, 0u);   // eight 16-bit running sums, two per word (<= TILE < 65536)
+    if (threadIdx.x == 0) {
 #pragma unroll
-        for (int w = 0; w < kSortWarps; ++w) {
-            uint4* p = reinterpret_cast<uint4*>(&S.cnt[w][kBinsPerThread * tid]);
-            uint4 v = *p;
-            v.x &= 0x07ff07ffu; v.y &= 0x07ff07ffu; v.z &= 0x07ff07ffu; v.w &= 0x07ff07ffu;
-            *p = run;
-            run.x += v.x; run.y += v.y; run.z += v.z; run.w += v.w;
-        }
-        tot[0] = run.x & 0xffffu; tot[1] = run.x >> 16; tot[2] = run.y & 0xffffu; tot[3] = run.y >> 16;
-        tot[4] = run.z & 0xffffu; tot[5] = run.z >> 16; tot[6] = run.w & 0xffffu; tot[7] = run.w >> 16;
-    }
-    unsigned* my_status = status + (size_t)tile * kSortBins + kBinsPerThread * tid;
-    {
-        const unsigned f = (tile > 0) ? kFlagAgg : kFlagIncl;   // tile 0: its totals are its inclusive prefixes
-        st_volatile_v4(my_status, make_uint4(f | tot[0], f | tot[1], f | tot[2], f | tot[3]));
-        st_volatile_v4(my_status + 4, make_uint4(f | tot[4], f | tot[5], f | tot[6], f | tot[7]));
-    }
-    unsigned loc[kBinsPerThread];   // position of the tile's first word of digit d inside the tile
-    {
-        unsigned run = 0;
-#pragma unroll
-        for (int q = 0; q < kBinsPerThread; ++q) { loc[q] = run; run += tot[q]; }
-        const unsigned off = block_exclusive_scan_256(run, S.scan_tmp);
-#pragma unroll
-        for (int q = 0; q < kBinsPerThread; ++q) loc[q] += off;
-        const uint4 add = make_uint4(loc[0] | (loc[1] << 16), loc[2] | (loc[3] << 16), loc[4] | (loc[5] << 16), loc[6] | (loc[7] << 16));
-#pragma unroll
-        for (int w = 0; w < kSortWarps; ++w) {
-            uint4* p = reinterpret_cast<uint4*>(&S.cnt[w][kBinsPerThread * tid]);
-            uint4 v = *p;
-            v.x += add.x; v.y += add.y; v.z += add.z; v.w += add.w;
-            *p = v;
-        }
-    }
-    __syncthreads();
-
-    // ---- reorder inside the tile (stable); the words leave the registers before the look-back -------------------
-#pragma unroll
-    for (int i = 0; i < ITEMS; ++i) {
-        const unsigned d = (unsigned)(key[i] >> dshift) & dmask;
-        S.stage[S.cnt[warp][d] + rank[i]] = key[i];
-    }
-
-    // ---- decoupled look-back over the preceding tiles, kLookW status rows in flight ------------------------------
-    unsigned excl[kBinsPerThread];
-#pragma unroll
-    for (int q = 0; q < kBinsPerThread; ++q) excl[q] = 0u;
-    if (tile > 0) {
-        unsigned pending = 0xffu;
-        long long t = tile - 1;
-        while (pending) {
-            uint4 a[kLookW], b[kLookW];
-#pragma unroll
-            for (int j = 0; j < kLookW; ++j) {
-                const long long tt = (t - j >= 0) ? t - j : 0;   // rows before tile 0 are never consumed (tile 0 posts inclusive prefixes)
-                const unsigned* row = status + (size_t)tt * kSortBins + kBinsPerThread * tid;
-                a[j] = ld_volatile_v4(row);
-                b[j] = ld_volatile_v4(row + 4);
-            }
-            int used = 0;
-#pragma unroll
-            for (int j = 0; j < kLookW; ++j) {
-                if (pending && used == j) {
-                    const unsigned v[kBinsPerThread] = {a[j].x, a[j].y, a[j].z, a[j].w, b[j].x, b[j].y, b[j].z, b[j].w};
-                    bool ready = true;
-#pragma unroll
-                    for (int q = 0; q < kBinsPerThread; ++q) ready = ready && (((pending >> q) & 1u) == 0u || (v[q] >> 30) != 0u);
-                    if (ready) {
-#pragma unroll
-                        for (int q = 0; q < kBinsPerThread; ++q) {
-                            if ((pending >> q) & 1u) {
-                                if (v[q] & kFlagIncl) { excl[q] += v[q] & 0x7fffffffu; pending &= ~(1u << q); }
-                                else excl[q] += v[q] & 0x3fffffffu;
-                            }
-                        }
-                        used = j + 1;
-                    }
-                }
-            }
-            t -= used;
-            if (used == 0) __nanosleep(32);
-        }
-    }
-    if (tile > 0) {
-        st_volatile_v4(my_status, make_uint4(kFlagIncl | (excl[0] + tot[0]), kFlagIncl | (excl[1] + tot[1]),
-                                             kFlagIncl | (excl[2] + tot[2]), kFlagIncl | (excl[3] + tot[3])));
-        st_volatile_v4(my_status + 4, make_uint4(kFlagIncl | (excl[4] + tot[4]), kFlagIncl | (excl[5] + tot[5]),
-                                                 kFlagIncl | (excl[6] + tot[6]), kFlagIncl | (excl[7] + tot[7])));
-    }
-    {
-        uint4* gb = reinterpret_cast<uint4*>(&S.gbase[kBinsPerThread * tid]);
-        gb[0] = make_uint4(hb[0] + excl[0] - loc[0], hb[1] + excl[1] - loc[1], hb[2] + excl[2] - loc[2], hb[3] + excl[3] - loc[3]);
-        gb[1] = make_uint4(hb[4] + excl[4] - loc[4], hb[5] + excl[5] - loc[5], hb[6] + excl[6] - loc[6], hb[7] + excl[7] - loc[7]);
-    }
-    __syncthreads();
-
-    // ---- write runs of equal digits -------------------------------------------------------------------------------
-#pragma unroll
-    for (int i = 0; i < ITEMS; ++i) {
-        const unsigned j = i * kSortThreads + tid;
-        const unsigned long long kk = S.stage[j];
-        const unsigned d = (unsigned)(kk >> dshift) & dmask;
-        const unsigned g = S.gbase[d] + j;
-        if ((long long)g < N) out[g] = kk;
+        for (int w = 1; w < kSortWarps; ++w) { inv = max(inv, red[0][w]); mx = max(mx, red[1][w]); }
+        atomicMax(&P.hdr->inv_kmin, inv);   // integer atomics: the result does not depend on their order
+        atomicMax(&P.hdr->kmax, mx);
     }
 }
 
-// =========================================================================================================
-// Fix-up: order the runs of equal prefixes by (full key, index); write the permutation (and the sorted keys).
-// =========================================================================================================
+// phases W (FIRST: words are built from the keys and stored) and H: digit histogram of this block's segment
+template <bool FIRST>
+__device__ __forceinline__ void sort_phase_hist(const SortParams& P, unsigned* hist, int bins, const SortPlan& pl, int pass,
+                                                const unsigned long long* in) {
+    const int seg = blockIdx.x;
+    if (seg >= P.nseg) return;
+    const int dshift = pl.ibits + pl.lo(pass);
+    const unsigned dmask = (1u << pl.w(pass)) - 1u;
+    for (int i = threadIdx.x; i < bins; i += kSortThreads) hist[i] = 0u;
+    __syncthreads();
+    const long long k0 = (long long)seg * P.tps * kSortTile;
+    long long k1 = k0 + P.tps * kSortTile;
+    if (k1 > P.N) k1 = P.N;
+    for (long long base = k0; base < k1; base += kSortThreads * kKeygenItems) {
+        unsigned long long w[kKeygenItems];
+#pragma unroll
+        for (int j = 0; j < kKeygenItems; ++j) {
+            const long long k = base + j * kSortThreads + threadIdx.x;
+            w[j] = (k < k1) ? __ldcg((FIRST ? P.keys : in) + k) : 0ull;
+        }
+#pragma unroll
+        for (int j = 0; j < kKeygenItems; ++j) {
+            const long long k = base + j * kSortThreads + threadIdx.x;
+            if (k < k1) {
+                if (FIRST) {
+                    w[j] = (((w[j] - pl.kmin) >> pl.shift) << pl.ibits) | (unsigned long long)k;
+                    P.bufA[k] = w[j];
+                }
+                if (pass < pl.passes) atomicAdd(&hist[(unsigned)(w[j] >> dshift) & dmask], 1u);
+            }
+        }
+    }
+    __syncthreads();
+    unsigned* row = P.seg_hist + (size_t)seg * kSortBins;
+    for (int i = threadIdx.x; i < bins; i += kSortThreads) row[i] = hist[i];
+}
+
+// phase S: seg_hist[seg][d] -> exclusive prefix over the segments; bin_tot[d] = total.  Block b owns the strip of
+// kScanStrip = 8 digit values 8b..8b+7 (one 32-byte sector per segment row): the strip is loaded in one round
+// trip, warp w scans column w in shared memory, the strip is stored back.
+__device__ __forceinline__ void sort_phase_scan(const SortParams& P, unsigned* strip /* [nseg][8] */, int bins) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    static_assert(kScanStrip == kSortWarps, "warp w scans column w of the strip");
+    for (int b = blockIdx.x; b < bins / kScanStrip; b += gridDim.x) {
+        for (int s = tid; s < P.nseg; s += kSortThreads) {
+            const uint4* row = reinterpret_cast<const uint4*>(P.seg_hist + (size_t)s * kSortBins + kScanStrip * b);
+            const uint4 v0 = __ldcg(row), v1 = __ldcg(row + 1);
+            reinterpret_cast<uint4*>(strip + 8 * s)[0] = v0;
+            reinterpret_cast<uint4*>(strip + 8 * s)[1] = v1;
+        }
+        __syncthreads();
+        {
+            unsigned carry = 0;
+            for (int s0 = 0; s0 < P.nseg; s0 += 32) {
+                const int s = s0 + lane;
+                const unsigned v = (s < P.nseg) ? strip[8 * s + warp] : 0u;
+                unsigned inc = v;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += t;
+                }
+                if (s < P.nseg) strip[8 * s + warp] = carry + inc - v;
+                carry += __shfl_sync(0xffffffffu, inc, 31);
+            }
+            if (lane == 0) P.bin_tot[kScanStrip * b + warp] = carry;
+        }
+        __syncthreads();
+        for (int s = tid; s < P.nseg; s += kSortThreads) {
+            uint4* row = reinterpret_cast<uint4*>(P.seg_hist + (size_t)s * kSortBins + kScanStrip * b);
+            row[0] = reinterpret_cast<const uint4*>(strip + 8 * s)[0];
+            row[1] = reinterpret_cast<const uint4*>(strip + 8 * s)[1];
+        }
+        __syncthreads();
+    }
+}
+
+// phase P: stable scatter of this block's segment by the digit of `pass`.
+// Tile = 256 threads x 16 words, loaded warp-striped (item i of warp w at tile base + w*512 + 32 i + lane), so the
+// order (warp, item, lane) is the order of the input.
+// Ranking: per warp and digit a 16-bit counter [tag:5 | count:11].  For every item the lanes stamp their lane
+// number on their digit's counter and read it back: if every lane finds its own stamp, all 32 digits of the item
+// are distinct (78 % of the items for uniformly distributed 11-bit digits) and the rank is simply the counter;
+// otherwise the lanes that share a digit find each other with one ballot per digit bit.  (Measured in round 1:
+// MATCH.ANY iterates over the distinct values of a warp, ~230 cycles for random digits; shared-memory atomics do
+// not return ranks in lane order.)
+template <int DB>
+__device__ __forceinline__ void sort_phase_scatter(const SortParams& P, SortSmem<DB>& S, const SortPlan& pl, int pass,
+                                                   const unsigned long long* in, unsigned long long* out) {
+    constexpr int BINS = SortSmem<DB>::BINS, BPT = SortSmem<DB>::BPT, WPT = BPT / 2;
+    const int seg = blockIdx.x;
+    if (seg >= P.nseg) return;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const long long N = P.N;
+    const int dshift = pl.ibits + pl.lo(pass);
+    const unsigned dmask = (1u << pl.w(pass)) - 1u;
+
+    // first global position of every digit for this segment: exclusive scan of the totals + the segment's offset
+    {
+        unsigned hb[BPT], of[BPT];
+        ldcg_words<BPT>(P.bin_tot + BPT * tid, hb);
+        ldcg_words<BPT>(P.seg_hist + (size_t)seg * kSortBins + BPT * tid, of);
+        unsigned run = 0;
+#pragma unroll
+        for (int q = 0; q < BPT; ++q) { const unsigned t = hb[q]; hb[q] = run; run += t; }
+        const unsigned off = block_exclusive_scan_256(run, S.scan_tmp);
+#pragma unroll
+        for (int q = 0; q < BPT; ++q) S.run[BPT * tid + q] = hb[q] + off + of[q];
+    }
+
+    const long long t0 = (long long)seg * P.tps;
+    long long t1 = t0 + P.tps;
+    if (t1 > P.tiles) t1 = P.tiles;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    unsigned long long key[kSortItems];
+    auto load_tile = [&](long long tile) {
+        const long long base = tile * kSortTile + (long long)warp * (32 * kSortItems);
+#pragma unroll
+        for (int i = 0; i < kSortItems; ++i) {
+            const long long k = base + 32 * i + lane;
+            key[i] = (k < N) ? __ldcg(in + k) : ~0ull;   // padding sorts last in every pass and is never written (position >= N)
+        }
+    };
+    load_tile(t0);
+    for (long long tile = t0; tile < t1; ++tile) {
+        // ---- clear the counters (the tile's words are in registers: loaded while the previous tile was written) ---
+        {
+            uint4* c = reinterpret_cast<uint4*>(&S.cnt[0][0]);
+            constexpr int kVec = kSortWarps * BINS * 2 / 16;
+            static_assert(kVec % kSortThreads == 0, "counter clearing");
+#pragma unroll
+            for (int i = 0; i < kVec / kSortThreads; ++i) c[i * kSortThreads + tid] = make_uint4(0u, 0u, 0u, 0u);
+        }
+        __syncthreads();
+
+        // ---- rank ---------------------------------------------------------------------------------------------
+        unsigned short rank[kSortItems];
+        volatile unsigned short* cw = S.cnt[warp];
+        if constexpr (DB > 9) {
+            // wide digits: most items have 32 distinct digits — stamp, read back, and only on a collision find the peers
+#pragma unroll
+            for (int i = 0; i < kSortItems; ++i) {
+                const unsigned d = (unsigned)(key[i] >> dshift) & dmask;
+                const unsigned c = cw[d] & 0x7ffu;
+                __syncwarp();
+                cw[d] = (unsigned short)((lane << 11) | c);
+                __syncwarp();
+                const bool own = (cw[d] >> 11) == (unsigned)lane;
+                if (__all_sync(0xffffffffu, own)) {
+                    rank[i] = (unsigned short)c;
+                    cw[d] = (unsigned short)(c + 1u);
+                } else {
+                    unsigned peers = 0xffffffffu;
+#pragma unroll
+                    for (int b = 0; b < DB; ++b) {
+                        const bool bit = (d >> b) & 1u;
+                        const unsigned vote = __ballot_sync(0xffffffffu, bit);
+                        peers &= bit ? vote : ~vote;
+                    }
+                    const unsigned lower = peers & lt_mask;
+                    rank[i] = (unsigned short)(c + __popc(lower));
+                    if (lower == 0u) cw[d] = (unsigned short)(c + __popc(peers));
+                }
+                __syncwarp();
+            }
+        } else {
+            // narrow digits: collisions are the rule — the lanes that share a digit find each other with one ballot per digit
+            // bit (register work, independent across the items), then the counters are bumped item by item
+            unsigned peers[kSortItems];
+#pragma unroll
+            for (int i = 0; i < kSortItems; ++i) {
+                const unsigned d = (unsigned)(key[i] >> dshift) & dmask;
+                unsigned pe = 0xffffffffu;
+#pragma unroll
+                for (int b = 0; b < DB; ++b) {
+                    const bool bit = (d >> b) & 1u;
+                    const unsigned vote = __ballot_sync(0xffffffffu, bit);
+                    pe &= bit ? vote : ~vote;
+                }
+                peers[i] = pe;
+            }
+#pragma unroll
+            for (int i = 0; i < kSortItems; ++i) {
+                const unsigned d = (unsigned)(key[i] >> dshift) & dmask;
+                const unsigned c = cw[d];
+                __syncwarp();
+                const unsigned lower = peers[i] & lt_mask;
+                rank[i] = (unsigned short)(c + __popc(lower));
+                if (lower == 0u) cw[d] = (unsigned short)(c + __popc(peers[i]));
+                __syncwarp();
+            }
+        }
+        __syncthreads();
+
+        // ---- thread t owns BPT digits: per-warp counts -> exclusive over warps, tile totals -----------------------
+        unsigned tot[BPT];
+        {
+            unsigned run[WPT];   // 16-bit running sums, two per word (<= kSortTile < 65536)
+#pragma unroll
+            for (int i = 0; i < WPT; ++i) run[i] = 0u;
+#pragma unroll
+            for (int w = 0; w < kSortWarps; ++w) {
+                unsigned* p = reinterpret_cast<unsigned*>(&S.cnt[w][BPT * tid]);
+                unsigned v[WPT];
+                ld_words<WPT>(p, v);
+                st_words<WPT>(p, run);
+#pragma unroll
+                for (int i = 0; i < WPT; ++i) run[i] += v[i] & 0x07ff07ffu;
+            }
+#pragma unroll
+            for (int i = 0; i < WPT; ++i) { tot[2 * i] = run[i] & 0xffffu; tot[2 * i + 1] = run[i] >> 16; }
+        }
+        {
+            unsigned loc[BPT];   // position of the tile's first word of digit d inside the tile
+            unsigned run = 0;
+#pragma unroll
+            for (int q = 0; q < BPT; ++q) { loc[q] = run; run += tot[q]; }
+            const unsigned off = block_exclusive_scan_256(run, S.scan_tmp);
+#pragma unroll
+            for (int q = 0; q < BPT; ++q) loc[q] += off;
+            unsigned add[WPT];
+#pragma unroll
+            for (int i = 0; i < WPT; ++i) add[i] = loc[2 * i] | (loc[2 * i + 1] << 16);
+#pragma unroll
+            for (int w = 0; w < kSortWarps; ++w) {
+                unsigned* p = reinterpret_cast<unsigned*>(&S.cnt[w][BPT * tid]);
+                unsigned v[WPT];
+                ld_words<WPT>(p, v);
+#pragma unroll
+                for (int i = 0; i < WPT; ++i) v[i] += add[i];
+                st_words<WPT>(p, v);
+            }
+#pragma unroll
+            for (int q = 0; q < BPT; ++q) {
+                const int d = BPT * tid + q;
+                const unsigned r = S.run[d];
+                S.gbase[d] = r - loc[q];
+                S.run[d] = r + tot[q];
+            }
+        }
+        __syncthreads();
+
+        // ---- reorder inside the tile (stable), then write runs of equal digits ---------------------------------
+#pragma unroll
+        for (int i = 0; i < kSortItems; ++i) {
+            const unsigned d = (unsigned)(key[i] >> dshift) & dmask;
+            S.stage[S.cnt[warp][d] + rank[i]] = key[i];
+        }
+        if (tile + 1 < t1) load_tile(tile + 1);   // in flight while this tile is written
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < kSortItems; ++i) {
+            const unsigned j = i * kSortThreads + tid;
+            const unsigned long long kk = S.stage[j];
+            const unsigned d = (unsigned)(kk >> dshift) & dmask;
+            const unsigned g = S.gbase[d] + j;
+            if ((long long)g < N) out[g] = kk;
+        }
+        __syncthreads();
+    }
+}
+
+// phase F: order the runs of equal prefixes by (full key, index); write the permutation (and the sorted keys).
+// Particles whose prefixes collide (the key bits below `shift` were not sorted) form short runs; the thread at the
+// head of a run orders it.  A run longer than kFixMaxRun raises the fallback flag.
 constexpr int kFixMaxRun = 32;
 
-__global__ void __launch_bounds__(256)
-mex_fixup_kernel(const unsigned long long* __restrict__ bufA, const unsigned long long* __restrict__ bufB,
-                 const unsigned long long* __restrict__ keys, long long N, SortHeader* __restrict__ hdr,
-                 unsigned* __restrict__ perm, unsigned long long* __restrict__ keys_sorted) {
-    const SortPlan pl = load_plan(hdr, N);
-    const unsigned long long* __restrict__ words = (pl.passes & 1) ? bufB : bufA;
-    const unsigned long long imask = (pl.ibits >= 64) ? ~0ull : ((1ull << pl.ibits) - 1ull);
-    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= N) return;
-    const unsigned long long w = words[p];
+constexpr int kFixItems = 8;   // positions per thread and step: the loads of a step are issued together
+
+__device__ __noinline__ void sort_fix_run(const SortParams& P, const SortPlan& pl, const unsigned long long* words,
+                                          long long p, unsigned long long w) {
+    const long long N = P.N;
+    const unsigned long long imask = (1ull << pl.ibits) - 1ull;
     const unsigned long long pre = w >> pl.ibits;
-    const bool run_left = pl.shift > 0 && p > 0 && (words[p - 1] >> pl.ibits) == pre;
-    const bool run_right = pl.shift > 0 && p + 1 < N && (words[p + 1] >> pl.ibits) == pre;
-    if (!run_left && !run_right) {
-        const unsigned i = (unsigned)(w & imask);
-        perm[p] = i;
-        if (keys_sorted) keys_sorted[p] = keys[i];
-        return;
-    }
-    if (run_left) return;   // the head of the run writes for all its members
     unsigned idx[kFixMaxRun];
     unsigned long long key[kFixMaxRun];
     int len = 0;
     while (p + len < N && len < kFixMaxRun) {
-        const unsigned long long v = (len == 0) ? w : words[p + len];
+        const unsigned long long v = (len == 0) ? w : __ldcg(words + p + len);
         if ((v >> pl.ibits) != pre) break;
         idx[len] = (unsigned)(v & imask);
         ++len;
     }
-    if (len == kFixMaxRun && p + len < N && (words[p + len] >> pl.ibits) == pre) {
-        atomicExch(&hdr->fallback, 1u);   // too long to order here: the fallback sort redoes the whole job
+    if (len == kFixMaxRun && p + len < N && (__ldcg(words + p + len) >> pl.ibits) == pre) {
+        atomicExch(&P.hdr->fallback, 1u);   // too long to order here: the fallback sort redoes the whole job
         return;
     }
-    for (int j = 0; j < len; ++j) key[j] = keys[idx[j]];
+    for (int j = 0; j < len; ++j) key[j] = __ldcg(P.keys + idx[j]);
     // stable insertion sort by the full key: members arrive in index order (the passes are stable)
     for (int j = 1; j < len; ++j) {
         const unsigned long long kj = key[j];
@@ -461,9 +537,175 @@ mex_fixup_kernel(const unsigned long long* __restrict__ bufA, const unsigned lon
         key[q + 1] = kj; idx[q + 1] = ij;
     }
     for (int j = 0; j < len; ++j) {
-        perm[p + j] = idx[j];
-        if (keys_sorted) keys_sorted[p + j] = key[j];
+        P.perm[p + j] = idx[j];
+        if (P.keys_sorted) P.keys_sorted[p + j] = key[j];
     }
+}
+
+// phase F1: particles alone in their prefix are final; the heads of runs are listed (in the words buffer the last pass
+// left free: any order, every head writes a range of its own) for phase F2.
+__device__ __forceinline__ void sort_phase_fixup(const SortParams& P, const SortPlan& pl, const unsigned long long* words,
+                                                 unsigned* heads) {
+    const long long N = P.N;
+    const int lane = threadIdx.x & 31;
+    const unsigned long long imask = (1ull << pl.ibits) - 1ull;   // ibits <= 31
+    const long long stride = (long long)gridDim.x * kSortThreads * kFixItems;
+    for (long long base = (long long)blockIdx.x * kSortThreads * kFixItems; base < N; base += stride) {
+        unsigned long long w[kFixItems], wl[kFixItems], wr[kFixItems];
+#pragma unroll
+        for (int j = 0; j < kFixItems; ++j) {
+            const long long p = base + j * kSortThreads + threadIdx.x;
+            w[j] = (p < N) ? __ldcg(words + p) : 0ull;
+            wl[j] = (p > 0 && p < N) ? __ldcg(words + p - 1) : ~0ull;
+            wr[j] = (p + 1 < N) ? __ldcg(words + p + 1) : ~0ull;
+        }
+        unsigned long long ks[kFixItems];
+        bool lone[kFixItems], head[kFixItems];
+#pragma unroll
+        for (int j = 0; j < kFixItems; ++j) {
+            const long long p = base + j * kSortThreads + threadIdx.x;
+            const unsigned long long pre = w[j] >> pl.ibits;
+            const bool run_left = pl.shift > 0 && p > 0 && (wl[j] >> pl.ibits) == pre;
+            const bool run_right = pl.shift > 0 && p + 1 < N && (wr[j] >> pl.ibits) == pre;
+            lone[j] = p < N && !run_left && !run_right;
+            head[j] = p < N && !run_left && run_right;
+            ks[j] = (lone[j] && P.keys_sorted) ? __ldcg(P.keys + (unsigned)(w[j] & imask)) : 0ull;
+        }
+        unsigned hm[kFixItems], nh = 0;
+#pragma unroll
+        for (int j = 0; j < kFixItems; ++j) {
+            const long long p = base + j * kSortThreads + threadIdx.x;
+            if (lone[j]) {
+                P.perm[p] = (unsigned)(w[j] & imask);
+                if (P.keys_sorted) P.keys_sorted[p] = ks[j];
+            }
+            hm[j] = __ballot_sync(0xffffffffu, head[j]);
+            nh += __popc(hm[j]);
+        }
+        if (nh) {   // warp-uniform: one atomic per warp and step
+            unsigned at = 0;
+            if (lane == 0) at = atomicAdd(&P.hdr->nheads, nh);
+            at = __shfl_sync(0xffffffffu, at, 0);
+#pragma unroll
+            for (int j = 0; j < kFixItems; ++j) {
+                if (head[j]) heads[at + __popc(hm[j] & ((1u << lane) - 1u))] = (unsigned)(base + j * kSortThreads + threadIdx.x);
+                at += __popc(hm[j]);
+            }
+        }
+    }
+}
+
+// phase F2: one thread per run.
+__device__ __forceinline__ void sort_phase_fixruns(const SortParams& P, const SortPlan& pl, const unsigned long long* words,
+                                                   const unsigned* heads) {
+    const unsigned n = __ldcg(&P.hdr->nheads);
+    const unsigned stride = gridDim.x * kSortThreads;
+    for (unsigned i = blockIdx.x * kSortThreads + threadIdx.x; i < n; i += stride) {
+        const long long p = __ldcg(heads + i);
+        sort_fix_run(P, pl, words, p, __ldcg(words + p));
+    }
+}
+
+// ---- single-wave sort: every phase in one cooperative launch ---------------------------------------------------
+constexpr int kSmallDB = kSortDigitBits;   // 11-bit digits, at most three passes
+constexpr int kLargeDB = 9;                // 9-bit digits, at most four passes over 36 prefix bits
+constexpr int kLargePrefixBits = 4 * kLargeDB;
+
+#ifdef ETICS_SORT_PROF
+#define ETICS_PROF() do { if (blockIdx.x == 0 && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); P.hdr->prof[prof_i++] = t_; } } while (0)
+#else
+#define ETICS_PROF() do {} while (0)
+#endif
+
+__global__ void __launch_bounds__(kSortThreads, 2)
+mex_sort_small_kernel(const __grid_constant__ SortParams P) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    SortSmem<kSmallDB>& S = *reinterpret_cast<SortSmem<kSmallDB>*>(smem_raw);
+    constexpr int BINS = SortSmem<kSmallDB>::BINS;
+    cg::grid_group grid = cg::this_grid();
+#ifdef ETICS_SORT_PROF
+    int prof_i = 0;
+#endif
+    ETICS_PROF();
+    sort_phase_keys(P, S.red);
+    ETICS_PROF();
+    grid.sync();
+    ETICS_PROF();
+    const SortPlan pl = load_plan(P.hdr, P.N, P.prefix_bits, P.digit_bits);
+    sort_phase_hist<true>(P, S.run, BINS, pl, 0, nullptr);
+    ETICS_PROF();
+    grid.sync();
+    ETICS_PROF();
+    for (int pass = 0; pass < pl.passes; ++pass) {   // pl is the same in every block: the barriers match
+        const unsigned long long* in = (pass & 1) ? P.bufB : P.bufA;
+        unsigned long long* out = (pass & 1) ? P.bufA : P.bufB;
+        if (pass > 0) {
+            sort_phase_hist<false>(P, S.run, BINS, pl, pass, in);
+            ETICS_PROF();
+            grid.sync();
+            ETICS_PROF();
+        }
+        sort_phase_scan(P, reinterpret_cast<unsigned*>(S.stage), BINS);
+        ETICS_PROF();
+        grid.sync();
+        ETICS_PROF();
+        sort_phase_scatter<kSmallDB>(P, S, pl, pass, in, out);
+        ETICS_PROF();
+        grid.sync();
+        ETICS_PROF();
+    }
+    const unsigned long long* words = (pl.passes & 1) ? P.bufB : P.bufA;
+    unsigned* heads = reinterpret_cast<unsigned*>((pl.passes & 1) ? P.bufA : P.bufB);
+    sort_phase_fixup(P, pl, words, heads);
+    ETICS_PROF();
+    grid.sync();
+    sort_phase_fixruns(P, pl, words, heads);
+    ETICS_PROF();
+}
+
+// ---- bandwidth-bound sort: one kernel per phase; a pass beyond the plan's last one returns at once -----------------
+__global__ void __launch_bounds__(kSortThreads)
+mex_sort_keys_kernel(const __grid_constant__ SortParams P) {
+    __shared__ unsigned long long red[2][kSortWarps];
+    sort_phase_keys(P, red);
+}
+
+__global__ void __launch_bounds__(kSortThreads)
+mex_sort_hist_kernel(const __grid_constant__ SortParams P, int pass) {
+    __shared__ unsigned hist[1 << kLargeDB];
+    const SortPlan pl = load_plan(P.hdr, P.N, P.prefix_bits, P.digit_bits);
+    if (pass > 0 && pass >= pl.passes) return;
+    if (pass == 0) sort_phase_hist<true>(P, hist, 1 << kLargeDB, pl, 0, nullptr);
+    else sort_phase_hist<false>(P, hist, 1 << kLargeDB, pl, pass, (pass & 1) ? P.bufB : P.bufA);
+}
+
+__global__ void __launch_bounds__(kSortThreads)
+mex_sort_scan_kernel(const __grid_constant__ SortParams P, int pass) {
+    __shared__ __align__(16) unsigned strip[kSortMaxSegs * kScanStrip];
+    const SortPlan pl = load_plan(P.hdr, P.N, P.prefix_bits, P.digit_bits);
+    if (pass >= pl.passes) return;
+    sort_phase_scan(P, strip, 1 << kLargeDB);
+}
+
+__global__ void __launch_bounds__(kSortThreads, 3)
+mex_sort_scatter_kernel(const __grid_constant__ SortParams P, int pass) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    SortSmem<kLargeDB>& S = *reinterpret_cast<SortSmem<kLargeDB>*>(smem_raw);
+    const SortPlan pl = load_plan(P.hdr, P.N, P.prefix_bits, P.digit_bits);
+    if (pass >= pl.passes) return;
+    sort_phase_scatter<kLargeDB>(P, S, pl, pass, (pass & 1) ? P.bufB : P.bufA, (pass & 1) ? P.bufA : P.bufB);
+}
+
+__global__ void __launch_bounds__(kSortThreads)
+mex_sort_fixup_kernel(const __grid_constant__ SortParams P) {
+    const SortPlan pl = load_plan(P.hdr, P.N, P.prefix_bits, P.digit_bits);
+    sort_phase_fixup(P, pl, (pl.passes & 1) ? P.bufB : P.bufA, reinterpret_cast<unsigned*>((pl.passes & 1) ? P.bufA : P.bufB));
+}
+
+__global__ void __launch_bounds__(kSortThreads)
+mex_sort_fixruns_kernel(const __grid_constant__ SortParams P) {
+    const SortPlan pl = load_plan(P.hdr, P.N, P.prefix_bits, P.digit_bits);
+    sort_phase_fixruns(P, pl, (pl.passes & 1) ? P.bufB : P.bufA, reinterpret_cast<const unsigned*>((pl.passes & 1) ? P.bufA : P.bufB));
 }
 
 // =========================================================================================================
@@ -542,80 +784,100 @@ mex_sort_fallback_kernel(const SortHeader* __restrict__ hdr, const unsigned long
 // ---------------------------------------------------------------------------------------------------------
 // Host side.
 // ---------------------------------------------------------------------------------------------------------
-constexpr long long kSortSmallN = 1ll << 22;   // below: 4096-word tiles (more tiles in flight); above: 8192-word tiles
+struct SortDevice { int small_blocks; int scatter_blocks; };   // resident blocks of the cooperative kernel / of the scatter kernel
 
-template <int ITEMS, int MINB>
-static cudaError_t radix_pass_set_attr() {
-    return cudaFuncSetAttribute(mex_radix_pass_kernel<ITEMS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)sizeof(SortSmem<ITEMS>));
+static cudaError_t sort_device(SortDevice* out) {
+    static std::mutex mu;
+    static SortDevice cached[64];
+    static bool have[64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev >= 0 && dev < 64 && have[dev]) { *out = cached[dev]; return cudaSuccess; }
+    SortDevice d{};
+    int per_sm = 0;
+    e = cudaFuncSetAttribute(mex_sort_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem<kSmallDB>));
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mex_sort_small_kernel, kSortThreads, sizeof(SortSmem<kSmallDB>));
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    d.small_blocks = device_sm_count() * per_sm;
+    if (d.small_blocks > kSortMaxSegs) d.small_blocks = kSortMaxSegs;
+    e = cudaFuncSetAttribute(mex_sort_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem<kLargeDB>));
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mex_sort_scatter_kernel, kSortThreads, sizeof(SortSmem<kLargeDB>));
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    d.scatter_blocks = device_sm_count() * per_sm;
+    if (dev >= 0 && dev < 64) { cached[dev] = d; have[dev] = true; }
+    *out = d;
+    return cudaSuccess;
 }
 
 cudaError_t mex_sort_init_device() {
-    static DeviceOnce once;
-    return once.run([] {
-        cudaError_t e = radix_pass_set_attr<16, 3>();
-        if (e != cudaSuccess) return e;
-        return radix_pass_set_attr<32, 2>();
-    });
-}
-
-template <int ITEMS, int MINB>
-static cudaError_t radix_passes_enqueue(unsigned long long* bufA, unsigned long long* bufB, long long N, SortHeader* hdr,
-                                        const unsigned* hist, unsigned* status, long long status_rows, cudaStream_t st) {
-    auto kern = mex_radix_pass_kernel<ITEMS, MINB>;
-    constexpr int TILE = kSortThreads * ITEMS;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)((N + TILE - 1) / TILE));
-    cfg.blockDim = dim3(kSortThreads);
-    cfg.dynamicSmemBytes = sizeof(SortSmem<ITEMS>);
-    cfg.stream = st;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    for (int pass = 0; pass < kSortMaxPasses; ++pass) {
-        cudaError_t e = cudaLaunchKernelEx(&cfg, kern, (const unsigned long long*)bufA, bufB, N, pass, hdr, hist, status, status_rows);
-        if (e != cudaSuccess) return e;
-    }
-    return cudaSuccess;
+    SortDevice d;
+    return sort_device(&d);
 }
 
 cudaError_t mex_sort_enqueue(const double* pos, const double* mass, long long N, const MexLayout& L, char* ws,
                              unsigned* perm_out, unsigned long long* keys_sorted_out, bool pack, cudaStream_t st,
                              cudaEvent_t ev_keygen) {
-    cudaError_t e = mex_sort_init_device();
+    SortDevice dv;
+    cudaError_t e = sort_device(&dv);
     if (e != cudaSuccess) return e;
-    SortHeader* hdr = reinterpret_cast<SortHeader*>(ws + L.off_hdr);
-    unsigned* hist = reinterpret_cast<unsigned*>(ws + L.off_hist);
-    unsigned* status = reinterpret_cast<unsigned*>(ws + L.off_status);
-    unsigned long long* keys = reinterpret_cast<unsigned long long*>(ws + L.off_keys);
-    unsigned long long* bufA = reinterpret_cast<unsigned long long*>(ws + L.off_wordsA);
-    unsigned long long* bufB = reinterpret_cast<unsigned long long*>(ws + L.off_wordsB);
-    unsigned* itmp = reinterpret_cast<unsigned*>(ws + L.off_itmp);
-    double2* pk = reinterpret_cast<double2*>(ws + L.off_pk);
-
-    e = cudaMemsetAsync(ws + L.off_zero, 0, L.zero_bytes, st);
+    SortParams P{};
+    P.pos = pos; P.mass = mass; P.N = N;
+    P.keys = reinterpret_cast<unsigned long long*>(ws + L.off_keys);
+    P.pk = pack ? reinterpret_cast<double2*>(ws + L.off_pk) : nullptr;
+    P.hdr = reinterpret_cast<SortHeader*>(ws + L.off_hdr);
+    P.bufA = reinterpret_cast<unsigned long long*>(ws + L.off_wordsA);
+    P.bufB = reinterpret_cast<unsigned long long*>(ws + L.off_wordsB);
+    P.seg_hist = reinterpret_cast<unsigned*>(ws + L.off_seghist);
+    P.bin_tot = reinterpret_cast<unsigned*>(ws + L.off_bintot);
+    P.perm = perm_out; P.keys_sorted = keys_sorted_out;
+    P.tiles = (N + kSortTile - 1) / kSortTile;
+    e = cudaMemsetAsync(ws + L.off_hdr, 0, sizeof(SortHeader), st);
     if (e != cudaSuccess) return e;
-    const long long per_block = 256 * kKeygenItems;
-    long long blocks = (N + per_block - 1) / per_block;
-    const long long cap = (long long)device_sm_count() * 8;
-    if (blocks > cap) blocks = cap;
-    if (pack) mex_keygen_kernel<true><<<(unsigned)blocks, 256, 0, st>>>(pos, mass, N, keys, pk, hdr);
-    else mex_keygen_kernel<false><<<(unsigned)blocks, 256, 0, st>>>(pos, nullptr, N, keys, nullptr, hdr);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    mex_pack_kernel<<<(unsigned)blocks, 256, 0, st>>>(keys, N, hdr, bufA, hist);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
+    if (P.tiles <= dv.small_blocks) {
+        // One tile per block: the whole sort is a single wave and latency-bound.  Everything in one cooperative launch,
+        // three passes of 11-bit digits.
+        P.tps = 1;
+        P.nseg = (int)P.tiles;
+        P.prefix_bits = kSortPrefixBits;
+        P.digit_bits = kSmallDB;
+        void* args[] = {&P};
+        int grid = (int)P.tiles < 128 ? 128 : (int)P.tiles;   // fewer blocks: cheaper grid barriers
+        if (grid > dv.small_blocks) grid = dv.small_blocks;
+        e = cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(mex_sort_small_kernel), dim3((unsigned)grid),
+                                        dim3(kSortThreads), args, sizeof(SortSmem<kSmallDB>), st);
+        if (e != cudaSuccess) return e;
+    } else {
+        // Bandwidth-bound: one kernel per phase, a block per segment of consecutive tiles (two waves of segments), four
+        // passes of 9-bit digits over 36 prefix bits — with 2048 digit values a tile of 4096 words would scatter runs of
+        // two words (N = 1e8: 1.41 ms per scatter against 0.66 ms), and fewer prefix bits leave more runs to the fix-up.
+        long long segs = 2ll * dv.scatter_blocks;
+        if (segs > kSortMaxSegs) segs = kSortMaxSegs;
+        P.tps = (P.tiles + segs - 1) / segs;
+        P.nseg = (int)((P.tiles + P.tps - 1) / P.tps);
+        P.prefix_bits = kLargePrefixBits;
+        P.digit_bits = kLargeDB;
+        const int wide = device_sm_count() * 8;
+        mex_sort_keys_kernel<<<wide, kSortThreads, 0, st>>>(P);
+        constexpr int kPasses = kLargePrefixBits / kLargeDB;
+        for (int pass = 0; pass < kPasses; ++pass) {
+            mex_sort_hist_kernel<<<P.nseg, kSortThreads, 0, st>>>(P, pass);
+            mex_sort_scan_kernel<<<(1 << kLargeDB) / kScanStrip, kSortThreads, 0, st>>>(P, pass);
+            mex_sort_scatter_kernel<<<P.nseg, kSortThreads, sizeof(SortSmem<kLargeDB>), st>>>(P, pass);
+        }
+        mex_sort_fixup_kernel<<<wide, kSortThreads, 0, st>>>(P);
+        mex_sort_fixruns_kernel<<<wide, kSortThreads, 0, st>>>(P);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
     if (ev_keygen) cudaEventRecord(ev_keygen, st);
-    if (N < kSortSmallN) e = radix_passes_enqueue<16, 3>(bufA, bufB, N, hdr, hist, status, L.sort_rows, st);
-    else e = radix_passes_enqueue<32, 2>(bufA, bufB, N, hdr, hist, status, L.sort_rows, st);
-    if (e != cudaSuccess) return e;
-    mex_fixup_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(bufA, bufB, keys, N, hdr, perm_out, keys_sorted_out);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    mex_sort_fallback_kernel<<<1, 1024, 0, st>>>(hdr, keys, N, bufA, bufB, perm_out, itmp, keys_sorted_out);
+    unsigned* itmp = reinterpret_cast<unsigned*>(ws + L.off_itmp);
+    mex_sort_fallback_kernel<<<1, 1024, 0, st>>>(P.hdr, P.keys, N, P.bufA, P.bufB, perm_out, itmp, keys_sorted_out);
     return cudaGetLastError();
 }
 
