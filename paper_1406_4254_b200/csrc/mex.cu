@@ -127,7 +127,6 @@ MexLayout make_mex_layout(long long N, int lmax) {
     L.off_pk = take((size_t)N * 32);
     L.off_rec = take((size_t)L.tiles * kRecFields * kMexTile * 8);
     L.off_idxT = take((size_t)L.tiles * kMexTile * 4);
-    L.off_pre = take((size_t)L.rows * L.chunks * 8);
     L.off_tot = take((size_t)L.rows * L.tiles * 8);
     L.total = o;
     return L;
@@ -151,27 +150,12 @@ __device__ __forceinline__ Rec load_rec(const double* __restrict__ rec_tile, int
     return p;
 }
 
-static __global__ void __launch_bounds__(256)
-mex_gather_kernel(const double2* __restrict__ pk, const unsigned* __restrict__ perm,
-                  long long N, long long tiles, double* __restrict__ rec, unsigned* __restrict__ idxT) {
-    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (gid >= tiles * kMexTile) return;
-    const long long tile = gid / kMexTile;
-    const int rem = (int)(gid - tile * kMexTile);
-    const int k = rem / kMexThreads, c = rem - k * kMexThreads;
-    const long long p = tile * kMexTile + (long long)c * kMexK + k;
-    double x = 1.0, y = 0.0, z = 0.0, mk = 0.0;
-    unsigned i = 0;
-    if (p < N) {
-        i = perm[p];
-        const double2 a = pk[2 * (size_t)i], b = pk[2 * (size_t)i + 1];
-        x = a.x; y = a.y; z = b.x; mk = b.y;
-    }
-    const Geom g = geometry(x, y, z);
-    double* b = rec + (size_t)tile * kRecFields * kMexTile + rem;
-    b[0 * kMexTile] = g.r; b[1 * kMexTile] = g.rinv; b[2 * kMexTile] = g.ct; b[3 * kMexTile] = g.st;
-    b[4 * kMexTile] = g.cp; b[5 * kMexTile] = g.sp; b[6 * kMexTile] = mk;
-    idxT[(size_t)tile * kMexTile + rem] = i;
+__device__ __forceinline__ Rec load_rec_cg(const double* rec_tile, int k, int c) {   // records written earlier by this kernel
+    const double* b = rec_tile + k * kMexThreads + c;
+    Rec p;
+    p.r = __ldcg(b + 0 * kMexTile); p.rinv = __ldcg(b + 1 * kMexTile); p.ct = __ldcg(b + 2 * kMexTile); p.st = __ldcg(b + 3 * kMexTile);
+    p.cp = __ldcg(b + 4 * kMexTile); p.sp = __ldcg(b + 5 * kMexTile); p.mass = __ldcg(b + 6 * kMexTile);
+    return p;
 }
 
 // =========================================================================================================
@@ -214,7 +198,8 @@ struct Angles {
     }
 };
 
-// moments of one particle into the running sums of group G (both directions): q[], pq[] have NS entries
+// moments of one particle into the UNWEIGHTED chunk sums of group G (both directions): q[], pq[] have NS entries.
+// m >= 1: sum of (m r^l st) u_lm {cos, sin} m phi;  m = 0: sum of (m r^l) u_l0.  mex_weight_sums applies W_lm once per chunk.
 template <int LMAX, int G>
 __device__ __forceinline__ void mex_agg_particle(const Rec& p, double* __restrict__ q, double* __restrict__ pq) {
     Angles<LMAX> a;
@@ -231,19 +216,36 @@ __device__ __forceinline__ void mex_agg_particle(const Rec& p, double* __restric
 #pragma unroll
         for (int l = m; l <= LMAX; ++l) {
             double u;
-            if (l == m) u = (m == 0) ? 1.0 : a.sp1[m];
+            if (l == m) u = (m == 0) ? 1.0 : a.sp1[m] * p.st;   // m >= 1: the chain carries st u_lm = Y_lm
             else if (l == m + 1) u = p.ct * u1;
             else u = fma(p.ct, u1, -mex_gamma(l, m) * u2);
             u2 = u1; u1 = u;
-            const double wy = (m == 0) ? mex_W(l, 0) * u : (mex_W(l, m) * p.st) * u;
-            const double tq = mq[l] * wy, tp = mp[l] * wy;
             if (m == 0) {
-                q[sb + l] += tq;
-                pq[sb + l] += tp;
+                q[sb + l] = fma(mq[l], u, q[sb + l]);
+                pq[sb + l] = fma(mp[l], u, pq[sb + l]);
             } else {
+                const double tq = mq[l] * u, tp = mp[l] * u;
                 const int s = sb + 2 * (l - m);
                 q[s] = fma(tq, a.cm[m], q[s]);       q[s + 1] = fma(tq, a.sm[m], q[s + 1]);
                 pq[s] = fma(tp, a.cm[m], pq[s]);     pq[s + 1] = fma(tp, a.sm[m], pq[s + 1]);
+            }
+        }
+    }
+}
+
+template <int LMAX, int G>
+__device__ __forceinline__ void mex_weight_sums(double* __restrict__ q, double* __restrict__ pq) {
+#pragma unroll
+    for (int m = 0; m <= LMAX; ++m) {
+        if (!mex_in_group(LMAX, G, m)) continue;
+        const int sb = mex_slot_base(LMAX, m);
+#pragma unroll
+        for (int l = m; l <= LMAX; ++l) {
+            if (m == 0) {
+                q[sb + l] *= mex_W(l, 0); pq[sb + l] *= mex_W(l, 0);
+            } else {
+                const int s = sb + 2 * (l - m);
+                q[s] *= mex_W(l, m); q[s + 1] *= mex_W(l, m); pq[s] *= mex_W(l, m); pq[s + 1] *= mex_W(l, m);
             }
         }
     }
@@ -292,31 +294,34 @@ __device__ __forceinline__ void mex_eval_particle(const Rec& p, double* __restri
             }
         }
         // ---- sums over the group's m at this level, then the own moment ------------------------------------
-        const double lct = double(l) * p.ct;
-        double aP = 0.0, aT = 0.0, aF = 0.0;
+        //   sum_m P_lm E_m          = u_l0 E_0 + st aU,                 aU = sum_{m>=1} u_lm E_m
+        //   sum_m (dP_lm/dth) E_m   = -l st u_l1 E_0 + l ct aU - aV,    aV = sum_{m>=1, m<l} c_lm u_{l-1,m} E_m
+        //   sum_m m U_lm F'_m       = aF                                 (all in units of h_lm; W_lm rides on the sums)
+        const double mus = mu * p.st;
+        double aU = 0.0, aV = 0.0, aF = 0.0, aP0 = 0.0, aT0 = 0.0;
 #pragma unroll
         for (int m = 0; m <= l; ++m) {
             if (!mex_in_group(LMAX, G, m)) continue;
             const int sb = mex_slot_base(LMAX, m);
             if (m == 0) {
                 const double e = s[sb + l];
-                aP = fma(u[0], e, aP);
-                if (l >= 1) aT = fma(-(double(l) * p.st) * ul1, e, aT);
+                aP0 = u[0] * e;
+                if (l >= 1) aT0 = (-(double(l) * p.st) * ul1) * e;
                 s[sb + l] = fma(mex_W(l, 0) * mu, u[0], e);
             } else {
                 const int i = sb + 2 * (l - m);
                 const double E = fma(s[i], a.cm[m], s[i + 1] * a.sm[m]);
                 const double F = fma(s[i + 1], mcm[m], -s[i] * msm[m]);
-                const double Y = p.st * u[m];
-                const double T = (m < l) ? fma(lct, u[m], -(double((l + m) * (l - m)) / double(2 * l - 1)) * u1[m]) : lct * u[m];
-                aP = fma(Y, E, aP);
-                aT = fma(T, E, aT);
+                aU = fma(u[m], E, aU);
                 aF = fma(u[m], F, aF);
-                const double t = (mex_W(l, m) * mu) * Y;
+                if (m < l) aV = fma((double((l + m) * (l - m)) / double(2 * l - 1)) * u1[m], E, aV);
+                const double t = (mex_W(l, m) * mus) * u[m];
                 s[i] = fma(t, a.cm[m], s[i]);
                 s[i + 1] = fma(t, a.sm[m], s[i + 1]);
             }
         }
+        const double aP = fma(p.st, aU, aP0);
+        const double aT = fma(double(l) * p.ct, aU, aT0 - aV);
         const double pa = rho * aP;
         sP += pa;
         sR = fma(FWD ? -double(l + 1) : double(l), pa, sR);
@@ -335,76 +340,109 @@ __device__ __forceinline__ void mex_eval_particle(const Rec& p, double* __restri
 }
 
 // =========================================================================================================
-// M4 + M5a: chunk aggregates and the tile-level exclusive scans.  A tile is ONE WARP: lane = chunk of kMexK
-// consecutive sorted particles (no block barrier anywhere; 1954 independent tiles at N = 10^6 keep every SM
-// sub-partition fed).  Shared memory: V[row][33] (row = slot of q, then slot of p).
-//   1. each lane sums the moments of its chunk in registers (next record prefetched while the current one is used);
-//   2. the sums go to V transposed; lane = row then runs the exclusive scan along the 32 chunks serially
-//      (q rows inside-out, p rows outside-in; the loads do not depend on the running sum, so the chain is 32 DADDs);
-//   3. V is copied to pre[tile][row][lane] (coalesced, immediate offsets), the row totals to tot[row][tile].
+// M3 + M4: gather into geometry records and tile totals of the moments.  A tile is ONE WARP: lane = chunk of kMexK
+// consecutive sorted particles (no block barrier anywhere).
+//   1. the lane reads its 8 permutation entries (32 contiguous bytes) and the 8 packed (x,y,z,m) sectors, computes the
+//      geometry and stores the records (field-major, chunk-transposed: coalesced) and the indices;
+//   2. per column group the lane sums the moments of its chunk in registers (records re-read through L2 for the
+//      groups after the first);
+//   3. the sums go to shared memory transposed (V[row][33]) and lane = row adds the 32 chunk sums in chunk order:
+//      tot[row][tile].  The chunk sums themselves are NOT stored: the evaluation kernel recomputes them (98-180 bytes
+//      per particle written and read back in round 1).
 // =========================================================================================================
 constexpr int kVStride = kMexThreads + 1;
 static_assert(kMexThreads == 32, "the MEX scan kernels use warp-sized tiles");
 
+// CG: the records were written earlier by the calling kernel (read them through L2, not the non-coherent path)
+template <int LMAX, int G, bool CG>
+__device__ __forceinline__ void mex_chunk_sums(const double* rec_tile, int c, double* __restrict__ q, double* __restrict__ pq) {
+    constexpr int NS = mex_group_slots(LMAX, G);
+#pragma unroll
+    for (int s = 0; s < NS; ++s) { q[s] = 0.0; pq[s] = 0.0; }
+    Rec p = CG ? load_rec_cg(rec_tile, 0, c) : load_rec(rec_tile, 0, c);
+#pragma unroll(LMAX <= 6 ? 1 : 2)
+    for (int k = 0; k < kMexK; ++k) {
+        const int kn = (k + 1 < kMexK) ? k + 1 : k;
+        const Rec nx = CG ? load_rec_cg(rec_tile, kn, c) : load_rec(rec_tile, kn, c);
+        mex_agg_particle<LMAX, G>(p, q, pq);
+        p = nx;
+    }
+    mex_weight_sums<LMAX, G>(q, pq);
+}
+
 template <int LMAX, int G>
-__device__ __forceinline__ void mex_aggregate_group(const double* __restrict__ rec_tile, double* V,
-                                                    double* __restrict__ pre_tile, double* __restrict__ tot,
-                                                    long long tiles, long long tile) {
+__device__ __forceinline__ void mex_totals_group(const double* rec_tile, double* V, double* __restrict__ tot,
+                                                 long long tiles, long long tile) {
     constexpr int NS = mex_group_slots(LMAX, G);
     constexpr int RB = mex_row_base(LMAX, G);
     constexpr int ROWS = 2 * NS;
     const int c = threadIdx.x;
     double q[NS], pq[NS];
-#pragma unroll
-    for (int s = 0; s < NS; ++s) { q[s] = 0.0; pq[s] = 0.0; }
-    Rec p = load_rec(rec_tile, 0, c);
-#pragma unroll(LMAX <= 6 ? 1 : 2)
-    for (int k = 0; k < kMexK; ++k) {
-        const Rec nx = load_rec(rec_tile, (k + 1 < kMexK) ? k + 1 : k, c);
-        mex_agg_particle<LMAX, G>(p, q, pq);
-        p = nx;
-    }
+    mex_chunk_sums<LMAX, G, true>(rec_tile, c, q, pq);
 #pragma unroll
     for (int s = 0; s < NS; ++s) { V[s * kVStride + c] = q[s]; V[(NS + s) * kVStride + c] = pq[s]; }
     __syncwarp();
     for (int row = c; row < ROWS; row += kMexThreads) {
-        double* v = V + row * kVStride;
-        double x[kMexThreads];
-#pragma unroll
-        for (int j = 0; j < kMexThreads; ++j) x[j] = v[j];
+        const double* v = V + row * kVStride;
         double run = 0.0;
         if (row < NS) {
 #pragma unroll
-            for (int j = 0; j < kMexThreads; ++j) { v[j] = run; run += x[j]; }
+            for (int j = 0; j < kMexThreads; ++j) run += v[j];
         } else {
 #pragma unroll
-            for (int j = kMexThreads - 1; j >= 0; --j) { v[j] = run; run += x[j]; }
+            for (int j = kMexThreads - 1; j >= 0; --j) run += v[j];
         }
         tot[(size_t)(RB + row) * tiles + tile] = run;
     }
-    __syncwarp();
-#pragma unroll
-    for (int row = 0; row < ROWS; ++row) pre_tile[(RB + row) * kMexThreads + c] = V[row * kVStride + c];
     __syncwarp();
 }
 
 template <int LMAX>
 __global__ void __launch_bounds__(kMexThreads)
-mex_aggregate_kernel(const double* __restrict__ rec, double* __restrict__ pre, double* __restrict__ tot, long long tiles) {
+mex_gather_totals_kernel(const double2* __restrict__ pk, const unsigned* __restrict__ perm, long long N, long long tiles,
+                         double* rec, unsigned* __restrict__ idxT, double* __restrict__ tot) {
     constexpr int MAXROWS = 2 * mex_max_group_slots(LMAX);
     __shared__ double V[MAXROWS * kVStride];
     const long long tile = blockIdx.x;
-    const double* rec_tile = rec + (size_t)tile * kRecFields * kMexTile;
-    double* pre_tile = pre + (size_t)tile * mex_total_rows(LMAX) * kMexThreads;
+    const int c = threadIdx.x;
+    double* rec_tile = rec + (size_t)tile * kRecFields * kMexTile;
+    const long long p0 = tile * kMexTile + (long long)c * kMexK;
+    unsigned idx[kMexK];
+    if (p0 + kMexK <= N) {
+        static_assert(kMexK % 4 == 0, "the permutation entries of a chunk are read as 16-byte vectors");
+#pragma unroll
+        for (int k = 0; k < kMexK; k += 4) {
+            const uint4 a = *reinterpret_cast<const uint4*>(perm + p0 + k);
+            idx[k] = a.x; idx[k + 1] = a.y; idx[k + 2] = a.z; idx[k + 3] = a.w;
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < kMexK; ++k) idx[k] = (p0 + k < N) ? perm[p0 + k] : 0xffffffffu;
+    }
+    double2 xy[kMexK], zm[kMexK];
+#pragma unroll
+    for (int k = 0; k < kMexK; ++k) {
+        const bool ok = p0 + k < N;
+        xy[k] = ok ? pk[2 * (size_t)idx[k]] : make_double2(1.0, 0.0);       // padding: a massless particle
+        zm[k] = ok ? pk[2 * (size_t)idx[k] + 1] : make_double2(0.0, 0.0);
+    }
+#pragma unroll
+    for (int k = 0; k < kMexK; ++k) {
+        const Geom g = geometry(xy[k].x, xy[k].y, zm[k].x);
+        double* b = rec_tile + k * kMexThreads + c;
+        b[0 * kMexTile] = g.r; b[1 * kMexTile] = g.rinv; b[2 * kMexTile] = g.ct; b[3 * kMexTile] = g.st;
+        b[4 * kMexTile] = g.cp; b[5 * kMexTile] = g.sp; b[6 * kMexTile] = zm[k].y;
+        idxT[(size_t)tile * kMexTile + k * kMexThreads + c] = (p0 + k < N) ? idx[k] : 0u;
+    }
     constexpr int NG = mex_num_groups(LMAX);
-    mex_aggregate_group<LMAX, 0>(rec_tile, V, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 1) mex_aggregate_group<LMAX, 1>(rec_tile, V, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 2) mex_aggregate_group<LMAX, 2>(rec_tile, V, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 3) mex_aggregate_group<LMAX, 3>(rec_tile, V, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 4) mex_aggregate_group<LMAX, 4>(rec_tile, V, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 5) mex_aggregate_group<LMAX, 5>(rec_tile, V, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 6) mex_aggregate_group<LMAX, 6>(rec_tile, V, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 7) mex_aggregate_group<LMAX, 7>(rec_tile, V, pre_tile, tot, tiles, tile);
+    mex_totals_group<LMAX, 0>(rec_tile, V, tot, tiles, tile);
+    if constexpr (NG > 1) mex_totals_group<LMAX, 1>(rec_tile, V, tot, tiles, tile);
+    if constexpr (NG > 2) mex_totals_group<LMAX, 2>(rec_tile, V, tot, tiles, tile);
+    if constexpr (NG > 3) mex_totals_group<LMAX, 3>(rec_tile, V, tot, tiles, tile);
+    if constexpr (NG > 4) mex_totals_group<LMAX, 4>(rec_tile, V, tot, tiles, tile);
+    if constexpr (NG > 5) mex_totals_group<LMAX, 5>(rec_tile, V, tot, tiles, tile);
+    if constexpr (NG > 6) mex_totals_group<LMAX, 6>(rec_tile, V, tot, tiles, tile);
+    if constexpr (NG > 7) mex_totals_group<LMAX, 7>(rec_tile, V, tot, tiles, tile);
 }
 
 // =========================================================================================================
@@ -470,16 +508,50 @@ mex_tilescan_kernel(double* __restrict__ tot, long long tiles, RowDirs rd) {
 // Shared memory: out[k][4][lane] (Phi, a_r, a_theta, a_phi of the lane's K particles; lane-private columns).
 // =========================================================================================================
 template <int LMAX, int G>
-__device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ rec_tile, double* sOut,
-                                                   const double* __restrict__ pre_tile, const double* __restrict__ tot,
-                                                   long long tiles, long long tile) {
+__device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ rec_tile, double* sOut, double* V,
+                                                   const double* __restrict__ tot, long long tiles, long long tile) {
     constexpr int NS = mex_group_slots(LMAX, G);
     constexpr int RB = mex_row_base(LMAX, G);
+    static_assert(NS <= kMexThreads, "one lane per row in the chunk scan");
     const int c = threadIdx.x;
     double s[NS];
-    // inside-out: q
+    // M5a: chunk sums (recomputed, never stored in HBM), then the exclusive scans along the 32 chunks of the tile in shared
+    // memory, lane = row, serial in chunk order (q rows inside-out, p rows outside-in; the loads do not depend on the
+    // running sum, so the chain is 32 DADDs).  The p prefixes wait in V while the forward walk runs.
+    {
+        double pq[NS];
+        mex_chunk_sums<LMAX, G, false>(rec_tile, c, s, pq);
 #pragma unroll
-    for (int i = 0; i < NS; ++i) s[i] = pre_tile[(RB + i) * kMexThreads + c] + tot[(size_t)(RB + i) * tiles + tile];
+        for (int i = 0; i < NS; ++i) V[i * kVStride + c] = s[i];
+        __syncwarp();
+        if (c < NS) {
+            double* v = V + c * kVStride;
+            double x[kMexThreads];
+#pragma unroll
+            for (int j = 0; j < kMexThreads; ++j) x[j] = v[j];
+            double run = tot[(size_t)(RB + c) * tiles + tile];   // the tile's exclusive prefix over the preceding tiles
+#pragma unroll
+            for (int j = 0; j < kMexThreads; ++j) { v[j] = run; run += x[j]; }
+        }
+        __syncwarp();
+#pragma unroll
+        for (int i = 0; i < NS; ++i) s[i] = V[i * kVStride + c];
+        __syncwarp();
+#pragma unroll
+        for (int i = 0; i < NS; ++i) V[i * kVStride + c] = pq[i];
+        __syncwarp();
+        if (c < NS) {
+            double* v = V + c * kVStride;
+            double x[kMexThreads];
+#pragma unroll
+            for (int j = 0; j < kMexThreads; ++j) x[j] = v[j];
+            double run = tot[(size_t)(RB + NS + c) * tiles + tile];
+#pragma unroll
+            for (int j = kMexThreads - 1; j >= 0; --j) { v[j] = run; run += x[j]; }
+        }
+        __syncwarp();
+    }
+    // inside-out: q
     {
         Rec p = load_rec(rec_tile, 0, c);
 #pragma unroll(LMAX <= 6 ? 1 : 2)   // two particles in flight per walk pay at lmax >= 7 (N = 1e8, lmax 8: 18.0 -> 16.4 ms)
@@ -496,8 +568,8 @@ __device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ re
     }
     // outside-in: p
 #pragma unroll
-    for (int i = 0; i < NS; ++i)
-        s[i] = pre_tile[(RB + NS + i) * kMexThreads + c] + tot[(size_t)(RB + NS + i) * tiles + tile];
+    for (int i = 0; i < NS; ++i) s[i] = V[i * kVStride + c];
+    __syncwarp();   // V is free for the next group
     {
         Rec p = load_rec(rec_tile, kMexK - 1, c);
 #pragma unroll(LMAX <= 6 ? 1 : 2)   // two particles in flight per walk pay at lmax >= 7 (N = 1e8, lmax 8: 18.0 -> 16.4 ms)
@@ -518,27 +590,29 @@ __device__ __forceinline__ void st_global_v4(double* p, double a, double b, doub
     asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
 }
 
+#ifndef ETICS_EVAL_MINB
+#define ETICS_EVAL_MINB 12
+#endif
 template <int LMAX>
-__global__ void __launch_bounds__(kMexThreads, LMAX <= 6 ? 12 : 8)
-mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__ idxT,
-                    const double* __restrict__ pre, const double* __restrict__ tot,
+__global__ void __launch_bounds__(kMexThreads, LMAX <= 6 ? ETICS_EVAL_MINB : 8)
+mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__ idxT, const double* __restrict__ tot,
                     long long tiles, long long N, double* __restrict__ out4) {
     __shared__ double sOut[kMexK * 4 * kMexThreads];
+    __shared__ double V[mex_max_group_slots(LMAX) * kVStride];
     const long long tile = blockIdx.x;
     const int c = threadIdx.x;
     const double* rec_tile = rec + (size_t)tile * kRecFields * kMexTile;
-    const double* pre_tile = pre + (size_t)tile * mex_total_rows(LMAX) * kMexThreads;
 #pragma unroll
     for (int i = 0; i < kMexK * 4; ++i) sOut[i * kMexThreads + c] = 0.0;   // lane-private column: no barrier needed
     constexpr int NG = mex_num_groups(LMAX);
-    mex_evaluate_group<LMAX, 0>(rec_tile, sOut, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 1) mex_evaluate_group<LMAX, 1>(rec_tile, sOut, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 2) mex_evaluate_group<LMAX, 2>(rec_tile, sOut, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 3) mex_evaluate_group<LMAX, 3>(rec_tile, sOut, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 4) mex_evaluate_group<LMAX, 4>(rec_tile, sOut, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 5) mex_evaluate_group<LMAX, 5>(rec_tile, sOut, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 6) mex_evaluate_group<LMAX, 6>(rec_tile, sOut, pre_tile, tot, tiles, tile);
-    if constexpr (NG > 7) mex_evaluate_group<LMAX, 7>(rec_tile, sOut, pre_tile, tot, tiles, tile);
+    mex_evaluate_group<LMAX, 0>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 1) mex_evaluate_group<LMAX, 1>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 2) mex_evaluate_group<LMAX, 2>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 3) mex_evaluate_group<LMAX, 3>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 4) mex_evaluate_group<LMAX, 4>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 5) mex_evaluate_group<LMAX, 5>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 6) mex_evaluate_group<LMAX, 6>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 7) mex_evaluate_group<LMAX, 7>(rec_tile, sOut, V, tot, tiles, tile);
 #pragma unroll 1
     for (int k = 0; k < kMexK; ++k) {
         const long long p = tile * kMexTile + (long long)c * kMexK + k;
@@ -583,14 +657,14 @@ cudaError_t mex_sort_launch(const double* pos, long long N, unsigned long long* 
 template <int LMAX>
 static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, double* acc, double* pot, cudaStream_t st,
                                     cudaEvent_t* ev) {
-    const double* rec = reinterpret_cast<const double*>(ws + L.off_rec);
-    const unsigned* idxT = reinterpret_cast<const unsigned*>(ws + L.off_idxT);
-    double* pre = reinterpret_cast<double*>(ws + L.off_pre);
+    double* rec = reinterpret_cast<double*>(ws + L.off_rec);
+    unsigned* idxT = reinterpret_cast<unsigned*>(ws + L.off_idxT);
     double* tot = reinterpret_cast<double*>(ws + L.off_tot);
-    mex_aggregate_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(rec, pre, tot, L.tiles);
+    mex_gather_totals_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(
+        reinterpret_cast<const double2*>(ws + L.off_pk), reinterpret_cast<const unsigned*>(ws + L.off_perm), N, L.tiles, rec, idxT, tot);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    if (ev) cudaEventRecord(ev[4], st);
+    if (ev) { cudaEventRecord(ev[3], st); cudaEventRecord(ev[4], st); }
     RowDirs rd{};
     rd.ng = mex_num_groups(LMAX);
     for (int g = 0; g < rd.ng; ++g) { rd.rb[g] = mex_row_base(LMAX, g); rd.ns[g] = mex_group_slots(LMAX, g); }
@@ -599,7 +673,7 @@ static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, d
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[5], st);
     double* out4 = reinterpret_cast<double*>(ws + L.off_pk);   // the packed inputs were consumed by the gather
-    mex_evaluate_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(rec, idxT, pre, tot, L.tiles, N, out4);
+    mex_evaluate_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(rec, idxT, tot, L.tiles, N, out4);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     mex_unpack_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(reinterpret_cast<const double2*>(out4), N, acc, pot);
@@ -658,13 +732,6 @@ static cudaError_t mex_force_enqueue(const double* pos, const double* mass, long
     cudaError_t e = mex_sort_enqueue(pos, mass, N, L, ws, idxA, nullptr, true, st, ev ? ev[1] : nullptr);
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[2], st);
-    const long long gthreads = L.tiles * kMexTile;
-    mex_gather_kernel<<<(unsigned)((gthreads + 255) / 256), 256, 0, st>>>(
-        reinterpret_cast<const double2*>(ws + L.off_pk), idxA, N, L.tiles, reinterpret_cast<double*>(ws + L.off_rec),
-        reinterpret_cast<unsigned*>(ws + L.off_idxT));
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    if (ev) cudaEventRecord(ev[3], st);
     if (lmax <= 6) return mex_scan_part0(L, ws, N, lmax, acc, pot, st, ev);
     if (lmax <= 8) return mex_scan_part1(L, ws, N, lmax, acc, pot, st, ev);
     if (lmax == 9) return mex_scan_part2(L, ws, N, lmax, acc, pot, st, ev);

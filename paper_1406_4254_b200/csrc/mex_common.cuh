@@ -30,7 +30,10 @@ struct SortHeader {
 
 // ---- scan geometry (mex.cu) --------------------------------------------------------------------------------
 constexpr int kMexThreads = 32;          // a scan tile is one warp: lane = chunk of kMexK consecutive sorted particles
-constexpr int kMexK = 8;
+#ifndef ETICS_MEX_K
+#define ETICS_MEX_K 8
+#endif
+constexpr int kMexK = ETICS_MEX_K;
 constexpr int kMexTile = kMexThreads * kMexK;
 constexpr int kRecFields = 8;            // r, 1/r, cos th, sin th, cos ph, sin ph, mass, (spare)
 
@@ -47,7 +50,7 @@ struct MexLayout {
     size_t off_perm;            // sorted order: perm[rank] = original index (4N)
     size_t off_itmp;            // second index buffer of the fallback sort (4N)
     size_t off_pk;              // (x, y, z, m) by original index, one 32-byte sector per particle; later the (Phi, a) records
-    size_t off_rec, off_idxT, off_pre, off_tot;
+    size_t off_rec, off_idxT, off_tot;
     size_t total;
 };
 

@@ -444,9 +444,12 @@ scf_accumulate_kernel(const double* __restrict__ pos, const double* __restrict__
     __syncthreads();
 
     for (long long pass = pass0; pass < pass1; ++pass) {
+        // Warps on one SM sub-partition (warp % 4) take the latency-bound feature phases and the FMA-bound accumulation in
+        // opposite orders, so that the fp64 pipe has work while the other half waits on shared memory and rsqrt chains.
+        const bool features_first = ((warp >> 2) & 1) == 0;
         phase0(pass + 2);     // writes G[pass&1] (last read by phase1(pass), before the previous barrier)
         prefetch(pass + 3);   // overwrites X[(pass+1)&1], consumed by this thread's phase0(pass+1) one iteration ago
-        phase1(pass + 1);     // reads G[(pass+1)&1] (written before the previous barrier), writes F[(pass+1)&1]
+        if (features_first) phase1(pass + 1);   // reads G[(pass+1)&1] (written before the previous barrier), writes F[(pass+1)&1]
         if (active) {         // reads F[pass&1] (written before the previous barrier)
             const double* F = sF + (size_t)(pass & 1) * fbuf;
             // single-group tables: code specialised per level (beta_n as immediates).  Multi-group tables run the generic
@@ -459,6 +462,7 @@ scf_accumulate_kernel(const double* __restrict__ pos, const double* __restrict__
                 default: if (FULL) acc_unit_level<4>(F, g, u, g.rep, my_rep, lane, acc); else acc_unit_steps<4, -1>(F, g, u, g.rep, my_rep, lane, acc); break;
             }
         }
+        if (!features_first) phase1(pass + 1);
         __syncthreads();
     }
 
