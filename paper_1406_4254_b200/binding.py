@@ -18,11 +18,12 @@ ETICS_OK = 0
 ETICS_ERR_ARG, ETICS_ERR_LIMIT, ETICS_ERR_ALIGN, ETICS_ERR_WORKSPACE, ETICS_ERR_CUDA = -1, -2, -3, -4, -5
 ETICS_MAX_LMAX, ETICS_MAX_NMAX = 10, 32
 ETICS_WS_SCF_COEFFS, ETICS_WS_SCF_FORCE, ETICS_WS_MEX_FORCE = 0, 1, 2
+ETICS_WHAT_BOTH, ETICS_WHAT_POTENTIAL, ETICS_WHAT_FORCE = 0, 1, 2
 
 # every symbol include/etics.h declares (tests check that the library exports all of them)
 EXPORTS = [
     "etics_status_string", "etics_init", "etics_workspace_bytes", "etics_scf_coeffs", "etics_scf_force",
-    "etics_mex_force", "etics_mex_sort", "etics_host_scratch_bytes", "etics_scf_full_host",
+    "etics_mex_force", "etics_scf_force_ex", "etics_mex_force_ex", "etics_mex_sort", "etics_host_scratch_bytes", "etics_scf_full_host",
     "etics_mex_full_host", "etics_mex_force_timed", "etics_probe_dfma", "etics_probe_copy",
 ]
 
@@ -58,6 +59,10 @@ def lib() -> C.CDLL:
     L.etics_scf_force.argtypes = [_vp, _ll, _i, _i, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
     L.etics_mex_force.restype = _i
     L.etics_mex_force.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _vp, _sz, _vp]
+    L.etics_scf_force_ex.restype = _i
+    L.etics_scf_force_ex.argtypes = [_vp, _ll, _i, _i, _vp, _vp, _i, _vp, _vp, _vp, _sz, _vp]
+    L.etics_mex_force_ex.restype = _i
+    L.etics_mex_force_ex.argtypes = [_vp, _vp, _ll, _i, _i, _vp, _vp, _vp, _sz, _vp]
     L.etics_mex_sort.restype = _i
     L.etics_mex_sort.argtypes = [_vp, _ll, _vp, _vp, _vp, _sz, _vp]
     L.etics_host_scratch_bytes.restype = _sz
@@ -162,7 +167,38 @@ def etics_mex_force(pos, mass, lmax: int, acc=None, pot=None, workspace=None, st
     return acc, pot
 
 
-MEX_STAGES = ("keygen", "radix_passes", "gather", "aggregate", "tilescan", "evaluate")
+def _opt(t, name):
+    return None if t is None else _dev(t, name)
+
+
+def etics_scf_force_ex(pos, nmax: int, lmax: int, A, B, what: int, acc=None, pot=None, stream=None):
+    """etics_scf_force with a selector: ETICS_WHAT_POTENTIAL returns (None, pot), ETICS_WHAT_FORCE returns (acc, None)."""
+    N = pos.shape[1]
+    if acc is None and what != ETICS_WHAT_POTENTIAL:
+        acc = torch.empty((3, N), dtype=torch.float64, device=pos.device)
+    if pot is None and what != ETICS_WHAT_FORCE:
+        pot = torch.empty(N, dtype=torch.float64, device=pos.device)
+    s = lib().etics_scf_force_ex(_dev(pos, "pos"), N, nmax, lmax, _dev(A, "A"), _dev(B, "B"), what, _opt(acc, "acc"),
+                                 _opt(pot, "pot"), None, 0, _stream(stream))
+    _check(s, "etics_scf_force_ex")
+    return (None if what == ETICS_WHAT_POTENTIAL else acc), (None if what == ETICS_WHAT_FORCE else pot)
+
+
+def etics_mex_force_ex(pos, mass, lmax: int, what: int, acc=None, pot=None, workspace=None, stream=None):
+    """etics_mex_force with a selector (see etics_scf_force_ex)."""
+    N = mass.shape[0]
+    if acc is None and what != ETICS_WHAT_POTENTIAL:
+        acc = torch.empty((3, N), dtype=torch.float64, device=pos.device)
+    if pot is None and what != ETICS_WHAT_FORCE:
+        pot = torch.empty(N, dtype=torch.float64, device=pos.device)
+    workspace, wsb = _workspace(ETICS_WS_MEX_FORCE, N, 0, lmax, pos.device, workspace)
+    s = lib().etics_mex_force_ex(_dev(pos, "pos"), _dev(mass, "mass"), N, lmax, what, _opt(acc, "acc"), _opt(pot, "pot"),
+                                 workspace.data_ptr(), wsb, _stream(stream))
+    _check(s, "etics_mex_force_ex")
+    return (None if what == ETICS_WHAT_POTENTIAL else acc), (None if what == ETICS_WHAT_FORCE else pot)
+
+
+MEX_STAGES = ("sort", "sort_fallback", "gather_totals", "unused", "tilescan", "evaluate")
 
 
 def etics_mex_force_timed(pos, mass, lmax: int, acc, pot, workspace, stream=None):

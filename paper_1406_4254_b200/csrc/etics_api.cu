@@ -61,24 +61,40 @@ etics_status etics_scf_coeffs(const double* pos, const double* mass, long long N
     return from_cuda(scf_coeffs_launch(pos, mass, N, nmax, lmax, A, B, workspace, static_cast<cudaStream_t>(stream)));
 }
 
-etics_status etics_scf_force(const double* pos, long long N, int nmax, int lmax, const double* A, const double* B,
-                             double* acc, double* pot, void* workspace, size_t workspace_bytes, void* stream) {
+etics_status etics_scf_force_ex(const double* pos, long long N, int nmax, int lmax, const double* A, const double* B,
+                                int what, double* acc, double* pot, void* workspace, size_t workspace_bytes, void* stream) {
     etics_status s = check_sizes(N, nmax, lmax);
     if (s != ETICS_OK) return s;
     (void)workspace; (void)workspace_bytes;   // this call needs no workspace; NULL / 0 are accepted
-    if (!pos || !A || !B || !acc || !pot) return ETICS_ERR_ARG;
+    if (what != ETICS_WHAT_BOTH && what != ETICS_WHAT_POTENTIAL && what != ETICS_WHAT_FORCE) return ETICS_ERR_ARG;
+    if (what == ETICS_WHAT_POTENTIAL) acc = nullptr;
+    if (what == ETICS_WHAT_FORCE) pot = nullptr;
+    if (!pos || !A || !B || (!acc && what != ETICS_WHAT_POTENTIAL) || (!pot && what != ETICS_WHAT_FORCE)) return ETICS_ERR_ARG;
     if (misaligned(pos) || misaligned(A) || misaligned(B) || misaligned(acc) || misaligned(pot)) return ETICS_ERR_ALIGN;
-    return from_cuda(scf_force_launch(pos, N, nmax, lmax, A, B, acc, pot, static_cast<cudaStream_t>(stream)));
+    return from_cuda(scf_force_launch(pos, N, nmax, lmax, A, B, what, acc, pot, static_cast<cudaStream_t>(stream)));
+}
+
+etics_status etics_scf_force(const double* pos, long long N, int nmax, int lmax, const double* A, const double* B,
+                             double* acc, double* pot, void* workspace, size_t workspace_bytes, void* stream) {
+    return etics_scf_force_ex(pos, N, nmax, lmax, A, B, ETICS_WHAT_BOTH, acc, pot, workspace, workspace_bytes, stream);
+}
+
+etics_status etics_mex_force_ex(const double* pos, const double* mass, long long N, int lmax,
+                                int what, double* acc, double* pot, void* workspace, size_t workspace_bytes, void* stream) {
+    etics_status s = check_sizes(N, 0, lmax);
+    if (s != ETICS_OK) return s;
+    if (what != ETICS_WHAT_BOTH && what != ETICS_WHAT_POTENTIAL && what != ETICS_WHAT_FORCE) return ETICS_ERR_ARG;
+    if (what == ETICS_WHAT_POTENTIAL) acc = nullptr;
+    if (what == ETICS_WHAT_FORCE) pot = nullptr;
+    if (!pos || !mass || !workspace || (!acc && what != ETICS_WHAT_POTENTIAL) || (!pot && what != ETICS_WHAT_FORCE)) return ETICS_ERR_ARG;
+    if (misaligned(pos) || misaligned(mass) || misaligned(acc) || misaligned(pot) || misaligned(workspace)) return ETICS_ERR_ALIGN;
+    if (workspace_bytes < etics_workspace_bytes(ETICS_WS_MEX_FORCE, N, 0, lmax)) return ETICS_ERR_WORKSPACE;
+    return from_cuda(mex_force_launch(pos, mass, N, lmax, what, acc, pot, workspace, static_cast<cudaStream_t>(stream)));
 }
 
 etics_status etics_mex_force(const double* pos, const double* mass, long long N, int lmax,
                              double* acc, double* pot, void* workspace, size_t workspace_bytes, void* stream) {
-    etics_status s = check_sizes(N, 0, lmax);
-    if (s != ETICS_OK) return s;
-    if (!pos || !mass || !acc || !pot || !workspace) return ETICS_ERR_ARG;
-    if (misaligned(pos) || misaligned(mass) || misaligned(acc) || misaligned(pot) || misaligned(workspace)) return ETICS_ERR_ALIGN;
-    if (workspace_bytes < etics_workspace_bytes(ETICS_WS_MEX_FORCE, N, 0, lmax)) return ETICS_ERR_WORKSPACE;
-    return from_cuda(mex_force_launch(pos, mass, N, lmax, acc, pot, workspace, static_cast<cudaStream_t>(stream)));
+    return etics_mex_force_ex(pos, mass, N, lmax, ETICS_WHAT_BOTH, acc, pot, workspace, workspace_bytes, stream);
 }
 
 etics_status etics_mex_sort(const double* pos, long long N, unsigned long long* keys_sorted, unsigned int* perm,

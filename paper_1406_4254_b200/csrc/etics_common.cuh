@@ -139,18 +139,15 @@ inline int device_sm_count() {
     return v;
 }
 
-// One __constant__ copy per translation unit (no relocatable device code needed).
+// One __constant__ copy per translation unit (no relocatable device code needed); uploaded by the unit's per-device init.
 #define ETICS_DEFINE_CONSTANTS()                                                                     \
     static __constant__ etics::BasisConstants c_basis;                                               \
-    static cudaError_t etics_upload_constants() {                                                    \
-        static etics::DeviceOnce once;                                                               \
-        return once.run([] {                                                                         \
-            etics::BasisConstants* host = new etics::BasisConstants;                                 \
-            etics::fill_basis_constants(*host);                                                      \
-            cudaError_t e = cudaMemcpyToSymbol(c_basis, host, sizeof(*host));                        \
-            delete host;                                                                             \
-            return e;                                                                                \
-        });                                                                                          \
+    static cudaError_t etics_upload_constants_now() {                                                \
+        etics::BasisConstants* host = new etics::BasisConstants;                                     \
+        etics::fill_basis_constants(*host);                                                          \
+        cudaError_t e = cudaMemcpyToSymbol(c_basis, host, sizeof(*host));                            \
+        delete host;                                                                                 \
+        return e;                                                                                    \
     }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -196,14 +193,14 @@ cudaError_t scf_init_constants();
 size_t scf_coeffs_workspace(long long N, int nmax, int lmax);
 cudaError_t scf_coeffs_launch(const double* pos, const double* mass, long long N, int nmax, int lmax,
                               double* A, double* B, void* ws, cudaStream_t st);
-cudaError_t scf_force_launch(const double* pos, long long N, int nmax, int lmax, const double* A, const double* B,
+cudaError_t scf_force_launch(const double* pos, long long N, int nmax, int lmax, const double* A, const double* B, int what,
                              double* acc, double* pot, cudaStream_t st);
 
 cudaError_t mex_init_constants();
 size_t mex_workspace(long long N, int lmax);
 cudaError_t mex_sort_launch(const double* pos, long long N, unsigned long long* keys_sorted, unsigned int* perm,
                             void* ws, cudaStream_t st);
-cudaError_t mex_force_launch(const double* pos, const double* mass, long long N, int lmax,
+cudaError_t mex_force_launch(const double* pos, const double* mass, long long N, int lmax, int what,
                              double* acc, double* pot, void* ws, cudaStream_t st);
 
 cudaError_t mex_force_timed(const double* pos, const double* mass, long long N, int lmax, double* acc, double* pot,

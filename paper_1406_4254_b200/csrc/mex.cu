@@ -257,7 +257,8 @@ __device__ __forceinline__ void mex_weight_sums(double* __restrict__ q, double* 
 //   BWD: s = p (exterior), radial factor r^l,      d/dr factor  l/r;      own moment m r^-(l+1)
 // Level by level: the m sums of a level (P, dP/dtheta, U-weighted) are formed first and meet the radial factor
 // once per level.  out[0..3] += (Phi, a_r, a_theta, a_phi) contributions.
-template <int LMAX, int G, bool FWD>
+// PO: potential only: the derivative sums are not formed.
+template <int LMAX, int G, bool FWD, bool PO>
 __device__ __forceinline__ void mex_eval_particle(const Rec& p, double* __restrict__ s, double* __restrict__ out) {
     Angles<LMAX> a;
     a.init(p);
@@ -306,27 +307,28 @@ __device__ __forceinline__ void mex_eval_particle(const Rec& p, double* __restri
             if (m == 0) {
                 const double e = s[sb + l];
                 aP0 = u[0] * e;
-                if (l >= 1) aT0 = (-(double(l) * p.st) * ul1) * e;
+                if (!PO && l >= 1) aT0 = (-(double(l) * p.st) * ul1) * e;
                 s[sb + l] = fma(mex_W(l, 0) * mu, u[0], e);
             } else {
                 const int i = sb + 2 * (l - m);
                 const double E = fma(s[i], a.cm[m], s[i + 1] * a.sm[m]);
-                const double F = fma(s[i + 1], mcm[m], -s[i] * msm[m]);
                 aU = fma(u[m], E, aU);
-                aF = fma(u[m], F, aF);
-                if (m < l) aV = fma((double((l + m) * (l - m)) / double(2 * l - 1)) * u1[m], E, aV);
+                if (!PO) aF = fma(u[m], fma(s[i + 1], mcm[m], -s[i] * msm[m]), aF);
+                if (!PO && m < l) aV = fma((double((l + m) * (l - m)) / double(2 * l - 1)) * u1[m], E, aV);
                 const double t = (mex_W(l, m) * mus) * u[m];
                 s[i] = fma(t, a.cm[m], s[i]);
                 s[i + 1] = fma(t, a.sm[m], s[i + 1]);
             }
         }
         const double aP = fma(p.st, aU, aP0);
-        const double aT = fma(double(l) * p.ct, aU, aT0 - aV);
         const double pa = rho * aP;
         sP += pa;
-        sR = fma(FWD ? -double(l + 1) : double(l), pa, sR);
-        sT = fma(rho, aT, sT);
-        sF = fma(rho, aF, sF);
+        if (!PO) {
+            const double aT = fma(double(l) * p.ct, aU, aT0 - aV);
+            sR = fma(FWD ? -double(l + 1) : double(l), pa, sR);
+            sT = fma(rho, aT, sT);
+            sF = fma(rho, aF, sF);
+        }
         rho *= FWD ? p.rinv : p.r;
         mu *= FWD ? p.r : p.rinv;
 #pragma unroll
@@ -334,9 +336,11 @@ __device__ __forceinline__ void mex_eval_particle(const Rec& p, double* __restri
             if (mex_in_group(LMAX, G, m)) { u2[m] = u1[m]; u1[m] = u[m]; }
     }
     out[0] -= sP;
-    out[1] = fma(p.rinv, sR, out[1]);
-    out[2] = fma(p.rinv, sT, out[2]);
-    out[3] = fma(p.rinv, sF, out[3]);
+    if (!PO) {
+        out[1] = fma(p.rinv, sR, out[1]);
+        out[2] = fma(p.rinv, sT, out[2]);
+        out[3] = fma(p.rinv, sF, out[3]);
+    }
 }
 
 // =========================================================================================================
@@ -507,7 +511,7 @@ mex_tilescan_kernel(double* __restrict__ tot, long long tiles, RowDirs rd) {
 // M5c + M6 + M7: walk, evaluate, transform, scatter.
 // Shared memory: out[k][4][lane] (Phi, a_r, a_theta, a_phi of the lane's K particles; lane-private columns).
 // =========================================================================================================
-template <int LMAX, int G>
+template <int LMAX, int G, bool PO>
 __device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ rec_tile, double* sOut, double* V,
                                                    const double* __restrict__ tot, long long tiles, long long tile) {
     constexpr int NS = mex_group_slots(LMAX, G);
@@ -560,7 +564,7 @@ __device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ re
             double o[4];
 #pragma unroll
             for (int j = 0; j < 4; ++j) o[j] = sOut[(k * 4 + j) * kMexThreads + c];
-            mex_eval_particle<LMAX, G, true>(p, s, o);
+            mex_eval_particle<LMAX, G, true, PO>(p, s, o);
 #pragma unroll
             for (int j = 0; j < 4; ++j) sOut[(k * 4 + j) * kMexThreads + c] = o[j];
             p = nx;
@@ -578,7 +582,7 @@ __device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ re
             double o[4];
 #pragma unroll
             for (int j = 0; j < 4; ++j) o[j] = sOut[(k * 4 + j) * kMexThreads + c];
-            mex_eval_particle<LMAX, G, false>(p, s, o);
+            mex_eval_particle<LMAX, G, false, PO>(p, s, o);
 #pragma unroll
             for (int j = 0; j < 4; ++j) sOut[(k * 4 + j) * kMexThreads + c] = o[j];
             p = nx;
@@ -593,7 +597,7 @@ __device__ __forceinline__ void st_global_v4(double* p, double a, double b, doub
 #ifndef ETICS_EVAL_MINB
 #define ETICS_EVAL_MINB 12
 #endif
-template <int LMAX>
+template <int LMAX, bool PO>
 __global__ void __launch_bounds__(kMexThreads, LMAX <= 6 ? ETICS_EVAL_MINB : 8)
 mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__ idxT, const double* __restrict__ tot,
                     long long tiles, long long N, double* __restrict__ out4) {
@@ -605,20 +609,24 @@ mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__
 #pragma unroll
     for (int i = 0; i < kMexK * 4; ++i) sOut[i * kMexThreads + c] = 0.0;   // lane-private column: no barrier needed
     constexpr int NG = mex_num_groups(LMAX);
-    mex_evaluate_group<LMAX, 0>(rec_tile, sOut, V, tot, tiles, tile);
-    if constexpr (NG > 1) mex_evaluate_group<LMAX, 1>(rec_tile, sOut, V, tot, tiles, tile);
-    if constexpr (NG > 2) mex_evaluate_group<LMAX, 2>(rec_tile, sOut, V, tot, tiles, tile);
-    if constexpr (NG > 3) mex_evaluate_group<LMAX, 3>(rec_tile, sOut, V, tot, tiles, tile);
-    if constexpr (NG > 4) mex_evaluate_group<LMAX, 4>(rec_tile, sOut, V, tot, tiles, tile);
-    if constexpr (NG > 5) mex_evaluate_group<LMAX, 5>(rec_tile, sOut, V, tot, tiles, tile);
-    if constexpr (NG > 6) mex_evaluate_group<LMAX, 6>(rec_tile, sOut, V, tot, tiles, tile);
-    if constexpr (NG > 7) mex_evaluate_group<LMAX, 7>(rec_tile, sOut, V, tot, tiles, tile);
+    mex_evaluate_group<LMAX, 0, PO>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 1) mex_evaluate_group<LMAX, 1, PO>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 2) mex_evaluate_group<LMAX, 2, PO>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 3) mex_evaluate_group<LMAX, 3, PO>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 4) mex_evaluate_group<LMAX, 4, PO>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 5) mex_evaluate_group<LMAX, 5, PO>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 6) mex_evaluate_group<LMAX, 6, PO>(rec_tile, sOut, V, tot, tiles, tile);
+    if constexpr (NG > 7) mex_evaluate_group<LMAX, 7, PO>(rec_tile, sOut, V, tot, tiles, tile);
 #pragma unroll 1
     for (int k = 0; k < kMexK; ++k) {
         const long long p = tile * kMexTile + (long long)c * kMexK + k;
         if (p >= N) continue;
-        const Rec r = load_rec(rec_tile, k, c);
         const unsigned i = idxT[(size_t)tile * kMexTile + k * kMexThreads + c];
+        if (PO) {   // out4 is the caller's pot array: one 8-byte store at the original index
+            out4[i] = sOut[(k * 4 + 0) * kMexThreads + c];
+            continue;
+        }
+        const Rec r = load_rec(rec_tile, k, c);
         Geom g;
         g.r = r.r; g.rinv = r.rinv; g.ct = r.ct; g.st = r.st; g.cp = r.cp; g.sp = r.sp;
         double ax, ay, az;
@@ -636,7 +644,7 @@ mex_unpack_kernel(const double2* __restrict__ out4, long long N, double* __restr
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const double2 a = out4[2 * i], b = out4[2 * i + 1];
-    pot[i] = a.x;
+    if (pot) pot[i] = a.x;   // null: force only
     acc[i] = a.y;
     acc[N + i] = b.x;
     acc[2 * N + i] = b.y;
@@ -655,7 +663,7 @@ cudaError_t mex_sort_launch(const double* pos, long long N, unsigned long long* 
 #endif   // ETICS_MEX_PART == 0
 
 template <int LMAX>
-static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, double* acc, double* pot, cudaStream_t st,
+static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, int what, double* acc, double* pot, cudaStream_t st,
                                     cudaEvent_t* ev) {
     double* rec = reinterpret_cast<double*>(ws + L.off_rec);
     unsigned* idxT = reinterpret_cast<unsigned*>(ws + L.off_idxT);
@@ -672,23 +680,29 @@ static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, d
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[5], st);
-    double* out4 = reinterpret_cast<double*>(ws + L.off_pk);   // the packed inputs were consumed by the gather
-    mex_evaluate_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(rec, idxT, tot, L.tiles, N, out4);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    mex_unpack_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(reinterpret_cast<const double2*>(out4), N, acc, pot);
-    e = cudaGetLastError();
+    if (what == ETICS_WHAT_POTENTIAL) {
+        mex_evaluate_kernel<LMAX, true><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(rec, idxT, tot, L.tiles, N, pot);
+        e = cudaGetLastError();
+    } else {
+        double* out4 = reinterpret_cast<double*>(ws + L.off_pk);   // the packed inputs were consumed by the gather
+        mex_evaluate_kernel<LMAX, false><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(rec, idxT, tot, L.tiles, N, out4);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        mex_unpack_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(reinterpret_cast<const double2*>(out4), N, acc,
+                                                                          what == ETICS_WHAT_FORCE ? nullptr : pot);
+        e = cudaGetLastError();
+    }
     if (ev) cudaEventRecord(ev[6], st);
     return e;
 }
 
 // The scan launch sequence of one lmax range per translation unit.
-#define ETICS_SCAN_ARGS const MexLayout &L, char *ws, long long N, int lmax, double *acc, double *pot, cudaStream_t st, cudaEvent_t *ev
+#define ETICS_SCAN_ARGS const MexLayout &L, char *ws, long long N, int lmax, int what, double *acc, double *pot, cudaStream_t st, cudaEvent_t *ev
 cudaError_t mex_scan_part0(ETICS_SCAN_ARGS);
 cudaError_t mex_scan_part1(ETICS_SCAN_ARGS);
 cudaError_t mex_scan_part2(ETICS_SCAN_ARGS);
 cudaError_t mex_scan_part3(ETICS_SCAN_ARGS);
-#define ETICS_CASE(LM) case LM: return mex_scan_enqueue<LM>(L, ws, N, acc, pot, st, ev);
+#define ETICS_CASE(LM) case LM: return mex_scan_enqueue<LM>(L, ws, N, what, acc, pot, st, ev);
 #if ETICS_MEX_PART == 0
 cudaError_t mex_scan_part0(ETICS_SCAN_ARGS) {
     switch (lmax) {
@@ -723,7 +737,7 @@ cudaError_t mex_scan_part3(ETICS_SCAN_ARGS) {
 #if ETICS_MEX_PART == 0
 // ev (optional): 7 events recorded at: start, after keygen, after the radix passes, after gather, after aggregate,
 // after tilescan, after evaluate.
-static cudaError_t mex_force_enqueue(const double* pos, const double* mass, long long N, int lmax,
+static cudaError_t mex_force_enqueue(const double* pos, const double* mass, long long N, int lmax, int what,
                                      double* acc, double* pot, void* wsv, cudaStream_t st, cudaEvent_t* ev) {
     const MexLayout L = make_mex_layout(N, lmax);
     char* ws = static_cast<char*>(wsv);
@@ -732,27 +746,28 @@ static cudaError_t mex_force_enqueue(const double* pos, const double* mass, long
     cudaError_t e = mex_sort_enqueue(pos, mass, N, L, ws, idxA, nullptr, true, st, ev ? ev[1] : nullptr);
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[2], st);
-    if (lmax <= 6) return mex_scan_part0(L, ws, N, lmax, acc, pot, st, ev);
-    if (lmax <= 8) return mex_scan_part1(L, ws, N, lmax, acc, pot, st, ev);
-    if (lmax == 9) return mex_scan_part2(L, ws, N, lmax, acc, pot, st, ev);
-    return mex_scan_part3(L, ws, N, lmax, acc, pot, st, ev);
+    if (lmax <= 6) return mex_scan_part0(L, ws, N, lmax, what, acc, pot, st, ev);
+    if (lmax <= 8) return mex_scan_part1(L, ws, N, lmax, what, acc, pot, st, ev);
+    if (lmax == 9) return mex_scan_part2(L, ws, N, lmax, what, acc, pot, st, ev);
+    return mex_scan_part3(L, ws, N, lmax, what, acc, pot, st, ev);
 }
 
-cudaError_t mex_force_launch(const double* pos, const double* mass, long long N, int lmax,
+cudaError_t mex_force_launch(const double* pos, const double* mass, long long N, int lmax, int what,
                              double* acc, double* pot, void* ws, cudaStream_t st) {
-    return mex_force_enqueue(pos, mass, N, lmax, acc, pot, ws, st, nullptr);
+    return mex_force_enqueue(pos, mass, N, lmax, what, acc, pot, ws, st, nullptr);
 }
 
 // Measurement support: the same launch sequence with CUDA events between the stages; synchronises the stream.
 cudaError_t mex_force_timed(const double* pos, const double* mass, long long N, int lmax, double* acc, double* pot,
                             void* ws, cudaStream_t st, float* stage_ms) {
-    cudaEvent_t ev[7];
-    for (auto& x : ev) { cudaError_t e = cudaEventCreate(&x); if (e != cudaSuccess) return e; }
-    cudaError_t e = mex_force_enqueue(pos, mass, N, lmax, acc, pot, ws, st, ev);
+    cudaEvent_t ev[7] = {};
+    cudaError_t e = cudaSuccess;
+    for (auto& x : ev) { e = cudaEventCreate(&x); if (e != cudaSuccess) break; }
+    if (e == cudaSuccess) e = mex_force_enqueue(pos, mass, N, lmax, ETICS_WHAT_BOTH, acc, pot, ws, st, ev);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e == cudaSuccess)
         for (int i = 0; i < 6; ++i) cudaEventElapsedTime(&stage_ms[i], ev[i], ev[i + 1]);
-    for (auto& x : ev) cudaEventDestroy(x);
+    for (auto& x : ev) if (x) cudaEventDestroy(x);
     return e;
 }
 

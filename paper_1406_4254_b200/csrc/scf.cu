@@ -17,7 +17,7 @@ namespace etics {
 
 ETICS_DEFINE_CONSTANTS()
 
-cudaError_t scf_init_constants() { return etics_upload_constants(); }
+cudaError_t scf_init_constants();
 
 // =========================================================================================================
 // Evaluation kernel (S6–S7).  One thread per particle; template on lmax so that every (l,m) array lives in
@@ -45,7 +45,10 @@ __host__ __device__ constexpr double leg_gamma_c(int l, int m) {
 
 // N1C > 0: nmax + 1 known at compile time (the n loops unroll fully and the compiler schedules across them);
 // N1C = 0: run-time nmax.
-template <int LMAX, int N1C>
+// PO: potential only ("faster since the derivatives ... are not calculated") — no C'_n chain, no
+// dP/dtheta, no U_lm sums, no transform; acc is not touched.  Otherwise both are computed; pot == nullptr (force only)
+// skips the store of the potential.
+template <int LMAX, int N1C, bool PO>
 __global__ void __launch_bounds__(eval_threads(LMAX), LMAX <= 6 ? ETICS_EVAL_MINBLOCKS : 1)
 scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
                 const double* __restrict__ A, const double* __restrict__ B,
@@ -124,10 +127,10 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
             for (int m = 0; m <= l; ++m) {
                 const double2 ab = tl[n * (l + 1) + m];
                 sa[m] = fma(ab.x, C, sa[m]);
-                sad[m] = fma(ab.x, D, sad[m]);
+                if (!PO) sad[m] = fma(ab.x, D, sad[m]);
                 if (m > 0) {
                     sb[m] = fma(ab.y, C, sb[m]);
-                    sbd[m] = fma(ab.y, D, sbd[m]);
+                    if (!PO) sbd[m] = fma(ab.y, D, sbd[m]);
                 }
             }
             // Q_{n+1} = xi Q_n - beta_{n+1} Q_{n-1};  Q'_{n+1} = xi Q'_n + Q_n - beta_{n+1} Q'_{n-1}
@@ -135,12 +138,12 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
             if (kMonicGeg) {
                 const double nb = -beta[n + 1];
                 Cn = fma(xi, C, nb * Cm);
-                Dn = fma(xi, D, fma(nb, Dm, C));
+                Dn = PO ? 0.0 : fma(xi, D, fma(nb, Dm, C));
             } else {
                 const double a = c_basis.geg_a[l][n + 1], b = c_basis.geg_b[l][n + 1];
                 const double ax = a * xi;
                 Cn = fma(ax, C, -b * Cm);
-                Dn = fma(ax, D, fma(a, C, -b * Dm));
+                Dn = PO ? 0.0 : fma(ax, D, fma(a, C, -b * Dm));
             }
             Cm = C; C = Cn; Dm = D; D = Dn;
         }
@@ -155,17 +158,17 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
             const double cmm = (m == 0) ? 1.0 : s_trig[(2 * m) * kEvalThreads];
             const double smm = (m == 0) ? 0.0 : s_trig[(2 * m + 1) * kEvalThreads];
             const double Ea = (m == 0) ? sa[0] : fma(sa[m], cmm, sb[m] * smm);
+            const double P = (m == 0) ? U0[0] : g.st * U0[m];
+            lv_p = fma(P, Ea, lv_p);
+            if (PO) continue;
             const double Ed = (m == 0) ? sad[0] : fma(sad[m], cmm, sbd[m] * smm);
-            double P, dP;
+            double dP;
             if (m == 0) {
-                P = U0[0];
                 dP = (l >= 1) ? -(double(l) * g.st) * U0[1] : 0.0;   // -P_l1 / h_l0, h_l1 / h_l0 = l
             } else {
-                P = g.st * U0[m];
                 // in monic terms U_{l-1,m} / h_lm = q_{l-1,m} (l-m)/(2l-1)
                 dP = (m < l) ? fma(lct, U0[m], -(double((l + m) * (l - m)) / double(2 * l - 1)) * U1[m]) : lct * U0[m];
             }
-            lv_p = fma(P, Ea, lv_p);
             lv_r = fma(P, Ed, lv_r);
             lv_t = fma(dP, Ea, lv_t);
             if (m > 0) {
@@ -174,21 +177,25 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
             }
         }
         s_pot = fma(fl, lv_p, s_pot);
-        s_r = fma(fl, fma(gl, lv_p, two_u2 * lv_r), s_r);
-        s_t = fma(fl, lv_t, s_t);
-        s_f = fma(fl, lv_f, s_f);
+        if (!PO) {
+            s_r = fma(fl, fma(gl, lv_p, two_u2 * lv_r), s_r);
+            s_t = fma(fl, lv_t, s_t);
+            s_f = fma(fl, lv_f, s_f);
+        }
         fl *= s;
         gl -= xr;
 #pragma unroll
         for (int m = 0; m <= l; ++m) { U2[m] = U1[m]; U1[m] = U0[m]; }
     }
 
-    double ax, ay, az;
-    to_cartesian(g, -s_r, -s_t * g.rinv, -s_f * g.rinv, ax, ay, az);
-    acc[k] = ax;
-    acc[N + k] = ay;
-    acc[2 * N + k] = az;
-    pot[k] = s_pot;
+    if (!PO) {
+        double ax, ay, az;
+        to_cartesian(g, -s_r, -s_t * g.rinv, -s_f * g.rinv, ax, ay, az);
+        acc[k] = ax;
+        acc[N + k] = ay;
+        acc[2 * N + k] = az;
+    }
+    if (PO || pot != nullptr) pot[k] = s_pot;
 }
 
 // =========================================================================================================
@@ -605,22 +612,14 @@ template <int LMAX>
 static cudaError_t launch_accumulate(const double* pos, const double* mass, long long N, const AccPlan& p, int bx,
                                      double* partial, cudaStream_t st) {
     const size_t smem = acc_smem_bytes(p);
-    static size_t smem_set[2] = {0, 0};   // per template instance
-    const bool full = p.ngroups == 1;
-    if (smem > smem_set[full]) {
-        cudaError_t e = full ? cudaFuncSetAttribute(scf_accumulate_kernel<LMAX, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
-                             : cudaFuncSetAttribute(scf_accumulate_kernel<LMAX, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        smem_set[full] = smem;
-    }
-    if (full) scf_accumulate_kernel<LMAX, true><<<dim3(bx, 1), kAccThreads, smem, st>>>(pos, mass, N, p, partial);
+    if (p.ngroups == 1) scf_accumulate_kernel<LMAX, true><<<dim3(bx, 1), kAccThreads, smem, st>>>(pos, mass, N, p, partial);
     else scf_accumulate_kernel<LMAX, false><<<dim3(bx, p.ngroups), kAccThreads, smem, st>>>(pos, mass, N, p, partial);
     return cudaGetLastError();
 }
 
 cudaError_t scf_coeffs_launch(const double* pos, const double* mass, long long N, int nmax, int lmax,
                               double* A, double* B, void* ws, cudaStream_t st) {
-    cudaError_t e = etics_upload_constants();
+    cudaError_t e = scf_init_constants();
     if (e != cudaSuccess) return e;
     const AccPlan p = make_acc_plan(N, nmax, lmax);
     double* partial = static_cast<double*>(ws);
@@ -638,41 +637,72 @@ cudaError_t scf_coeffs_launch(const double* pos, const double* mass, long long N
     return cudaGetLastError();
 }
 
-template <int LMAX, int N1C>
+// nmax = 10 (the paper's cut-off) at lmax <= 6 gets fully unrolled n loops: 166.5 -> 149 us at N = 1e6.
+// (20,10) with compile-time nmax and the n loops unrolled by 3: 6.41 -> 6.08 ms at N = 1e7 (fully unrolled — 5544
+// FMAs of straight-line code — it was slower, 8.5 ms).
+template <int LMAX>
+constexpr int eval_n1c(int nmax) { return (LMAX <= 6 && nmax == 10) ? 11 : (LMAX == 10 && nmax == 20) ? 21 : 0; }
+
+template <int LMAX, int N1C, bool PO>
 static cudaError_t launch_eval_n(const double* pos, long long N, int nmax, const double* A, const double* B,
                                  double* acc, double* pot, cudaStream_t st) {
-    auto kern = scf_eval_kernel<LMAX, N1C>;
     constexpr int kEvalThreads = eval_threads(LMAX);
     const size_t smem = (size_t)(nmax + 1) * num_lm(LMAX) * sizeof(double2) + (size_t)(2 * LMAX + 2) * kEvalThreads * sizeof(double);
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
     const long long blocks = (N + kEvalThreads - 1) / kEvalThreads;
-    kern<<<(unsigned)blocks, kEvalThreads, smem, st>>>(pos, N, nmax, A, B, acc, pot);
+    scf_eval_kernel<LMAX, N1C, PO><<<(unsigned)blocks, kEvalThreads, smem, st>>>(pos, N, nmax, A, B, acc, pot);
     return cudaGetLastError();
 }
 
-template <int LMAX>
+template <int LMAX, bool PO>
 static cudaError_t launch_eval(const double* pos, long long N, int nmax, const double* A, const double* B,
                                double* acc, double* pot, cudaStream_t st) {
-    // nmax = 10 (the paper's cut-off) at lmax <= 6 gets fully unrolled n loops: 166.5 -> 149 us at N = 1e6.
-    // (20,10) with compile-time nmax and the n loops unrolled by 3: 6.41 -> 6.08 ms at N = 1e7 (fully unrolled — 5544
-    // FMAs of straight-line code — it was slower, 8.5 ms).
-    if (LMAX <= 6 && nmax == 10) return launch_eval_n<LMAX, (LMAX <= 6 ? 11 : 0)>(pos, N, nmax, A, B, acc, pot, st);
-    if (LMAX == 10 && nmax == 20) return launch_eval_n<LMAX, (LMAX == 10 ? 21 : 0)>(pos, N, nmax, A, B, acc, pot, st);
-    return launch_eval_n<LMAX, 0>(pos, N, nmax, A, B, acc, pot, st);
+    if (LMAX <= 6 && nmax == 10) return launch_eval_n<LMAX, (LMAX <= 6 ? 11 : 0), PO>(pos, N, nmax, A, B, acc, pot, st);
+    if (LMAX == 10 && nmax == 20) return launch_eval_n<LMAX, (LMAX == 10 ? 21 : 0), PO>(pos, N, nmax, A, B, acc, pot, st);
+    return launch_eval_n<LMAX, 0, PO>(pos, N, nmax, A, B, acc, pot, st);
 }
 
-cudaError_t scf_force_launch(const double* pos, long long N, int nmax, int lmax, const double* A, const double* B,
+// what: ETICS_WHAT_BOTH | ETICS_WHAT_POTENTIAL (acc untouched) | ETICS_WHAT_FORCE (pot untouched)
+cudaError_t scf_force_launch(const double* pos, long long N, int nmax, int lmax, const double* A, const double* B, int what,
                              double* acc, double* pot, cudaStream_t st) {
-    cudaError_t e = etics_upload_constants();
+    cudaError_t e = scf_init_constants();
     if (e != cudaSuccess) return e;
+    if (what == ETICS_WHAT_FORCE) pot = nullptr;
     switch (lmax) {
-#define ETICS_CASE(LM) case LM: return launch_eval<LM>(pos, N, nmax, A, B, acc, pot, st);
+#define ETICS_CASE(LM) case LM: return what == ETICS_WHAT_POTENTIAL ? launch_eval<LM, true>(pos, N, nmax, A, B, acc, pot, st) \
+                                                                     : launch_eval<LM, false>(pos, N, nmax, A, B, acc, pot, st);
         ETICS_CASE(0) ETICS_CASE(1) ETICS_CASE(2) ETICS_CASE(3) ETICS_CASE(4) ETICS_CASE(5)
         ETICS_CASE(6) ETICS_CASE(7) ETICS_CASE(8) ETICS_CASE(9) ETICS_CASE(10)
 #undef ETICS_CASE
         default: return cudaErrorInvalidValue;
     }
+}
+
+// ---- per-device set-up: constants and the dynamic shared-memory limit of every kernel instance, once per device ----------
+constexpr int kMaxDynSmem = 227 * 1024;
+
+template <int LM>
+static cudaError_t set_kernel_attributes() {
+    cudaError_t e = cudaSuccess;
+    auto set = [&](auto kern) {
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
+    };
+    set(scf_accumulate_kernel<LM, true>);
+    set(scf_accumulate_kernel<LM, false>);
+    set(scf_eval_kernel<LM, 0, false>);
+    set(scf_eval_kernel<LM, 0, true>);
+    if constexpr (LM <= 6) { set(scf_eval_kernel<LM, 11, false>); set(scf_eval_kernel<LM, 11, true>); }
+    if constexpr (LM == 10) { set(scf_eval_kernel<LM, 21, false>); set(scf_eval_kernel<LM, 21, true>); }
+    if constexpr (LM > 0) { if (e == cudaSuccess) e = set_kernel_attributes<LM - 1>(); }
+    return e;
+}
+
+cudaError_t scf_init_constants() {
+    static DeviceOnce once;
+    return once.run([] {
+        cudaError_t e = etics_upload_constants_now();
+        if (e != cudaSuccess) return e;
+        return set_kernel_attributes<kMaxL>();
+    });
 }
 
 }  // namespace etics

@@ -219,3 +219,32 @@ def test_config3_full_size(E):
     the streaming oracle covers every particle in a few seconds."""
     pos, mass = W.config_particles(3)
     check_mex(E, pos, mass, 6)
+
+
+@pytest.mark.parametrize("lmax", [0, 3, 6, 8, 10])
+def test_force_only_and_potential_only(E, lmax):
+    """PAPER.md:213 ("force, potential or both"): the selector variants against the oracle and against the 'both' call."""
+    pos, mass = W.particles("hernquist", 4_321, seed=5, axes=(1.0, 0.8, 0.6))
+    dpos, dmass = dev(pos), dev(mass)
+    acc, pot = E.etics_mex_force(dpos, dmass, lmax)
+    sentinel = -12345.0
+    acc_p = torch.full_like(acc, sentinel)
+    pot_f = torch.full_like(pot, sentinel)
+    _, pot_p = E.etics_mex_force_ex(dpos, dmass, lmax, E.ETICS_WHAT_POTENTIAL)
+    acc_f, _ = E.etics_mex_force_ex(dpos, dmass, lmax, E.ETICS_WHAT_FORCE)
+    ws = torch.empty(E.etics_workspace_bytes(E.ETICS_WS_MEX_FORCE, pos.shape[1], 0, lmax), dtype=torch.uint8, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    assert E.lib().etics_mex_force_ex(dpos.data_ptr(), dmass.data_ptr(), pos.shape[1], lmax, E.ETICS_WHAT_POTENTIAL,
+                                      acc_p.data_ptr(), pot_p.data_ptr(), ws.data_ptr(), ws.numel(), st) == 0
+    assert E.lib().etics_mex_force_ex(dpos.data_ptr(), dmass.data_ptr(), pos.shape[1], lmax, E.ETICS_WHAT_FORCE,
+                                      acc_f.data_ptr(), pot_f.data_ptr(), ws.data_ptr(), ws.numel(), st) == 0
+    torch.cuda.synchronize()
+    assert torch.all(acc_p == sentinel) and torch.all(pot_f == sentinel)
+    acc0, pot0 = oracle.mex_force(pos, mass, lmax)
+    assert rel_err_scalar(pot_p.cpu().numpy(), pot0, floor=0.0) <= TOL
+    if lmax > 0:
+        assert rel_err_vector(acc_f.cpu().numpy(), acc0) <= TOL
+    assert torch.equal(acc_f, acc)
+    assert rel_err_scalar(pot_p.cpu().numpy(), pot.cpu().numpy(), floor=0.0) <= 1e-14
+    assert E.lib().etics_mex_force_ex(dpos.data_ptr(), dmass.data_ptr(), pos.shape[1], lmax, 7,
+                                      acc.data_ptr(), pot.data_ptr(), ws.data_ptr(), ws.numel(), st) == E.ETICS_ERR_ARG

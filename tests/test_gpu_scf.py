@@ -175,3 +175,33 @@ def test_config2_full_size_sampled(E):
     assert rel_err_vector(acc[:, idx], acc0) <= TOL
     assert np.all(np.isfinite(acc)) and np.all(np.isfinite(pot))
     assert abs(A[0] - 303.0 / 301.0) < 4 * 0.7048 / np.sqrt(n)
+
+
+@pytest.mark.parametrize("nmax,lmax", [(10, 6), (7, 3), (20, 10), (10, 8), (0, 0)])
+def test_force_only_and_potential_only(E, nmax, lmax):
+    """PAPER.md:253 ("force, potential or both"): the selector variants against the oracle, and bit-identical to the
+    corresponding outputs of the 'both' call; the array that is not asked for is not touched."""
+    pos, mass = W.particles("hernquist", 5_003, seed=7, axes=(1.0, 0.9, 0.7))
+    dpos, dmass = dev(pos), dev(mass)
+    A, B = E.etics_scf_coeffs(dpos, dmass, nmax, lmax)
+    acc, pot = E.etics_scf_force(dpos, nmax, lmax, A, B)
+    sentinel = -12345.0
+    acc_p = torch.full_like(acc, sentinel)
+    _, pot_p = E.etics_scf_force_ex(dpos, nmax, lmax, A, B, E.ETICS_WHAT_POTENTIAL, acc=None)
+    pot_f = torch.full_like(pot, sentinel)
+    acc_f, _ = E.etics_scf_force_ex(dpos, nmax, lmax, A, B, E.ETICS_WHAT_FORCE, pot=None)
+    # arrays passed but not asked for stay untouched
+    E.lib().etics_scf_force_ex(dpos.data_ptr(), pos.shape[1], nmax, lmax, A.data_ptr(), B.data_ptr(), E.ETICS_WHAT_POTENTIAL,
+                               acc_p.data_ptr(), pot_p.data_ptr(), None, 0, torch.cuda.current_stream().cuda_stream)
+    E.lib().etics_scf_force_ex(dpos.data_ptr(), pos.shape[1], nmax, lmax, A.data_ptr(), B.data_ptr(), E.ETICS_WHAT_FORCE,
+                               acc_f.data_ptr(), pot_f.data_ptr(), None, 0, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert torch.all(acc_p == sentinel) and torch.all(pot_f == sentinel)
+    A0, B0 = oracle.scf_coeffs(pos, mass, nmax, lmax)
+    acc0, pot0 = oracle.scf_force(pos, nmax, lmax, A0, B0)
+    assert rel_err_scalar(pot_p.cpu().numpy(), pot0, floor=0.0) <= TOL
+    assert rel_err_vector(acc_f.cpu().numpy(), acc0) <= TOL
+    assert torch.equal(acc_f, acc)
+    assert rel_err_scalar(pot_p.cpu().numpy(), pot.cpu().numpy(), floor=0.0) <= 1e-14   # same sums, possibly another schedule
+    assert E.lib().etics_scf_force_ex(dpos.data_ptr(), pos.shape[1], nmax, lmax, A.data_ptr(), B.data_ptr(), 3,
+                                      acc.data_ptr(), pot.data_ptr(), None, 0, 0) == E.ETICS_ERR_ARG
