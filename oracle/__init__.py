@@ -153,3 +153,31 @@ def mex_force_at(pos, mass, lmax: int, sample_idx, threads: int = 0):
     if rc != 0:
         raise ValueError(f"oracle_mex_force_at failed: {rc}")
     return acc, pot
+
+
+def leapfrog(force, pos, vel, dt: float, nsteps: int):
+    """Kick-drift-kick leapfrog of x'' = a(x) (§3.4: the systems are evolved with a leapfrog that calls the
+    force routine once per step), written out step by step:
+        v += (dt/2) a(x);  x += dt v;  a = force(x);  v += (dt/2) a(x)
+    force(pos) -> acc, both (3, N).  Returns (pos, vel, acc) after nsteps steps; the inputs are not modified."""
+    x = _f64(pos).copy(); v = _f64(vel).copy()
+    a = force(x)
+    for _ in range(nsteps):
+        v = v + (0.5 * dt) * a
+        x = x + dt * v
+        a = force(x)
+        v = v + (0.5 * dt) * a
+    return x, v, a
+
+
+def scf_acceleration(mass, nmax: int, lmax: int):
+    """force(pos) for leapfrog(): the SCF full force calculation on the particles themselves."""
+    def f(x):
+        A, B = scf_coeffs(x, mass, nmax, lmax)
+        return scf_force(x, nmax, lmax, A, B)[0]
+    return f
+
+
+def mex_acceleration(mass, lmax: int):
+    """force(pos) for leapfrog(): the MEX full force calculation."""
+    return lambda x: mex_force(x, mass, lmax)[0]

@@ -25,6 +25,7 @@ EXPORTS = [
     "etics_status_string", "etics_init", "etics_workspace_bytes", "etics_scf_coeffs", "etics_scf_force",
     "etics_mex_force", "etics_scf_force_ex", "etics_mex_force_ex", "etics_mex_sort", "etics_host_scratch_bytes", "etics_scf_full_host",
     "etics_mex_full_host", "etics_mex_force_timed", "etics_probe_dfma", "etics_probe_copy",
+    "etics_stepper_workspace_bytes", "etics_stepper_create", "etics_stepper_step", "etics_stepper_destroy",
 ]
 
 _lib = None
@@ -73,6 +74,14 @@ def lib() -> C.CDLL:
     L.etics_mex_full_host.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _vp, _sz, _vp]
     L.etics_mex_force_timed.restype = _i
     L.etics_mex_force_timed.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _vp, _sz, _vp, C.POINTER(C.c_float)]
+    L.etics_stepper_workspace_bytes.restype = _sz
+    L.etics_stepper_workspace_bytes.argtypes = [_i, _ll, _i, _i]
+    L.etics_stepper_create.restype = _i
+    L.etics_stepper_create.argtypes = [C.POINTER(_vp), _i, _vp, _vp, _vp, _ll, _i, _i, C.c_double, _vp, _vp, _vp, _sz, _i, _vp]
+    L.etics_stepper_step.restype = _i
+    L.etics_stepper_step.argtypes = [_vp, _i]
+    L.etics_stepper_destroy.restype = _i
+    L.etics_stepper_destroy.argtypes = [_vp]
     L.etics_probe_dfma.restype = _i
     L.etics_probe_dfma.argtypes = [_i, _vp, C.POINTER(C.c_double), _vp]
     L.etics_probe_copy.restype = _i
@@ -266,3 +275,35 @@ def etics_probe_copy(dst, src, stream=None) -> int:
     s = lib().etics_probe_copy(dst.data_ptr(), src.data_ptr(), nbytes, _stream(stream))
     _check(s, "etics_probe_copy")
     return 2 * nbytes
+
+
+class Stepper:
+    """Handle of etics_stepper_* (include/etics.h): kick-drift-kick steps with the SCF (method 0) or MEX (method 1) force.
+    pos, vel are updated in place; acc, pot hold the acceleration / potential at the current positions."""
+
+    def __init__(self, method: int, pos, vel, mass, dt: float, nmax: int = 0, lmax: int = 0, use_graph: bool = True, stream=None):
+        N = mass.shape[0]
+        self.pos, self.vel, self.mass = pos, vel, mass
+        self.acc = torch.empty((3, N), dtype=torch.float64, device=pos.device)
+        self.pot = torch.empty(N, dtype=torch.float64, device=pos.device)
+        self.workspace = torch.empty(lib().etics_stepper_workspace_bytes(method, N, nmax, lmax), dtype=torch.uint8, device=pos.device)
+        h = _vp()
+        s = lib().etics_stepper_create(C.byref(h), method, _dev(pos, "pos"), _dev(vel, "vel"), _dev(mass, "mass"), N, nmax, lmax,
+                                       float(dt), _dev(self.acc, "acc"), _dev(self.pot, "pot"), self.workspace.data_ptr(),
+                                       self.workspace.numel(), int(bool(use_graph)), _stream(stream))
+        _check(s, "etics_stepper_create")
+        self._h = h
+
+    def step(self, nsteps: int = 1) -> None:
+        _check(lib().etics_stepper_step(self._h, nsteps), "etics_stepper_step")
+
+    def close(self) -> None:
+        if self._h is not None:
+            _check(lib().etics_stepper_destroy(self._h), "etics_stepper_destroy")
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
