@@ -25,7 +25,7 @@ EXPORTS = [
     "etics_status_string", "etics_init", "etics_workspace_bytes", "etics_scf_coeffs", "etics_scf_force",
     "etics_mex_force", "etics_scf_force_ex", "etics_mex_force_ex", "etics_mex_sort", "etics_host_scratch_bytes", "etics_scf_full_host",
     "etics_mex_full_host", "etics_mex_force_timed", "etics_probe_dfma", "etics_probe_copy",
-    "etics_stepper_workspace_bytes", "etics_stepper_create", "etics_stepper_step", "etics_stepper_destroy",
+    "etics_step_host_scratch_bytes", "etics_step_host", "etics_stepper_workspace_bytes", "etics_stepper_create", "etics_stepper_step", "etics_stepper_destroy",
 ]
 
 _lib = None
@@ -74,6 +74,10 @@ def lib() -> C.CDLL:
     L.etics_mex_full_host.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _vp, _sz, _vp]
     L.etics_mex_force_timed.restype = _i
     L.etics_mex_force_timed.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _vp, _sz, _vp, C.POINTER(C.c_float)]
+    L.etics_step_host_scratch_bytes.restype = _sz
+    L.etics_step_host_scratch_bytes.argtypes = [_ll, _i, _i, _i]
+    L.etics_step_host.restype = _i
+    L.etics_step_host.argtypes = [_vp, _vp, _ll, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp, _vp]
     L.etics_stepper_workspace_bytes.restype = _sz
     L.etics_stepper_workspace_bytes.argtypes = [_i, _ll, _i, _i]
     L.etics_stepper_create.restype = _i
@@ -260,6 +264,22 @@ def etics_mex_full_host(pos_h, mass_h, lmax: int, acc_h, pot_h, scratch, stream=
                                   _host(acc_h, "acc_h"), _host(pot_h, "pot_h"),
                                   scratch.data_ptr(), scratch.numel() * scratch.element_size(), _stream(stream))
     _check(s, "etics_mex_full_host")
+
+
+def etics_step_host_scratch_bytes(N: int, nmax: int, lmax: int, mex_lmax: int) -> int:
+    return lib().etics_step_host_scratch_bytes(N, nmax, lmax, mex_lmax)
+
+
+def etics_step_host(pos_h, mass_h, nmax: int, lmax: int, mex_lmax: int, acc_scf_h, pot_scf_h, acc_mex_h, pot_mex_h, scratch,
+                    A_h=None, B_h=None, stream=None, copy_stream=None):
+    """One upload, SCF + MEX full force calculations, results to host buffers; copy_stream (a torch stream) overlaps the copies."""
+    N = mass_h.shape[0]
+    s = lib().etics_step_host(_host(pos_h, "pos_h"), _host(mass_h, "mass_h"), N, nmax, lmax, mex_lmax,
+                              None if A_h is None else _host(A_h, "A_h"), None if B_h is None else _host(B_h, "B_h"),
+                              _host(acc_scf_h, "acc_scf_h"), _host(pot_scf_h, "pot_scf_h"), _host(acc_mex_h, "acc_mex_h"),
+                              _host(pot_mex_h, "pot_mex_h"), scratch.data_ptr(), scratch.numel() * scratch.element_size(),
+                              _stream(stream), None if copy_stream is None else _stream(copy_stream))
+    _check(s, "etics_step_host")
 
 
 def etics_probe_dfma(iters: int, sink, stream=None) -> float:

@@ -177,6 +177,93 @@ etics_status etics_mex_full_host(const double* pos_h, const double* mass_h, long
     return ETICS_OK;
 }
 
+// ---- one upload, both methods, overlapped copies ------------------------------------------------------------------------
+// Scratch layout: pos[3N] | mass[N] | acc_scf[3N] | pot_scf[N] | acc_mex[3N] | pot_mex[N] | A[T] | B[T] | ws_scf | ws_mex.
+size_t etics_step_host_scratch_bytes(long long N, int nmax, int lmax, int mex_lmax) {
+    if (check_sizes(N, nmax, lmax) != ETICS_OK || check_sizes(N, 0, mex_lmax) != ETICS_OK) return 0;
+    const size_t T = (size_t)(nmax + 1) * num_lm(lmax);
+    return 2 * (seg(3 * (size_t)N) + seg((size_t)N)) + seg(3 * (size_t)N) + seg((size_t)N) + 2 * seg(T) +
+           etics_workspace_bytes(ETICS_WS_SCF_COEFFS, N, nmax, lmax) + etics_workspace_bytes(ETICS_WS_MEX_FORCE, N, 0, mex_lmax);
+}
+
+etics_status etics_step_host(const double* pos_h, const double* mass_h, long long N, int nmax, int lmax, int mex_lmax,
+                             double* A_h, double* B_h, double* acc_scf_h, double* pot_scf_h, double* acc_mex_h, double* pot_mex_h,
+                             void* device_scratch, size_t scratch_bytes, void* stream, void* copy_stream) {
+    etics_status s = check_sizes(N, nmax, lmax);
+    if (s != ETICS_OK) return s;
+    s = check_sizes(N, 0, mex_lmax);
+    if (s != ETICS_OK) return s;
+    if (!pos_h || !mass_h || !acc_scf_h || !pot_scf_h || !acc_mex_h || !pot_mex_h || !device_scratch) return ETICS_ERR_ARG;
+    if (misaligned(device_scratch)) return ETICS_ERR_ALIGN;
+    if (scratch_bytes < etics_step_host_scratch_bytes(N, nmax, lmax, mex_lmax)) return ETICS_ERR_WORKSPACE;
+    if (etics_init() != ETICS_OK) return ETICS_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaStream_t cs = copy_stream ? static_cast<cudaStream_t>(copy_stream) : st;
+    const bool two = cs != st;
+    const size_t T = (size_t)(nmax + 1) * num_lm(lmax), n = (size_t)N;
+    char* p = static_cast<char*>(device_scratch);
+    double* d_pos = reinterpret_cast<double*>(p); p += seg(3 * n);
+    double* d_mass = reinterpret_cast<double*>(p); p += seg(n);
+    double* d_acc1 = reinterpret_cast<double*>(p); p += seg(3 * n);
+    double* d_pot1 = reinterpret_cast<double*>(p); p += seg(n);
+    double* d_acc2 = reinterpret_cast<double*>(p); p += seg(3 * n);
+    double* d_pot2 = reinterpret_cast<double*>(p); p += seg(n);
+    double* d_A = reinterpret_cast<double*>(p); p += seg(T);
+    double* d_B = reinterpret_cast<double*>(p); p += seg(T);
+    void* ws_scf = p; p += etics_workspace_bytes(ETICS_WS_SCF_COEFFS, N, nmax, lmax);
+    void* ws_mex = p;
+    const size_t ws_mex_bytes = etics_workspace_bytes(ETICS_WS_MEX_FORCE, N, 0, mex_lmax);
+
+    // events order the two streams; they are destroyed right after the enqueue (CUDA releases them once they have completed)
+    constexpr int kMaxChunks = 8;
+    cudaEvent_t ev[kMaxChunks + 4] = {};
+    int nev = 0;
+    bool ok = true;
+    auto fail = [&]() { ok = false; };
+    auto link = [&](cudaStream_t from, cudaStream_t to) {   // `to` continues after everything enqueued so far on `from`
+        if (!two || !ok) return;
+        cudaEvent_t e = nullptr;
+        if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return fail();
+        ev[nev++] = e;
+        if (cudaEventRecord(e, from) != cudaSuccess || cudaStreamWaitEvent(to, e, 0) != cudaSuccess) fail();
+    };
+    auto copy = [&](void* dst, const void* src, size_t bytes, cudaMemcpyKind kind) {
+        if (ok && bytes && cudaMemcpyAsync(dst, src, bytes, kind, cs) != cudaSuccess) fail();
+    };
+    link(st, cs);   // the copies start after the work already on the caller's stream
+
+    // H2D in ranges of whole accumulation blocks; each range is accumulated as soon as it has arrived (coefficients
+    // are additive over particles), so the upload hides the coefficient pass
+    long long per_block = 0;
+    const int blocks = scf_coeffs_blocks(N, nmax, lmax, &per_block);
+    const int chunks = !two ? 1 : (blocks < kMaxChunks ? blocks : kMaxChunks);
+    for (int c = 0; c < chunks && ok; ++c) {
+        const int b0 = (int)((long long)blocks * c / chunks), b1 = (int)((long long)blocks * (c + 1) / chunks);
+        const size_t k0 = (size_t)b0 * per_block;
+        size_t k1 = (size_t)b1 * per_block;
+        if (k1 > n || c == chunks - 1) k1 = n;
+        for (int d = 0; d < 3; ++d) copy(d_pos + d * n + k0, pos_h + d * n + k0, (k1 - k0) * 8, cudaMemcpyHostToDevice);
+        copy(d_mass + k0, mass_h + k0, (k1 - k0) * 8, cudaMemcpyHostToDevice);
+        link(cs, st);
+        if (ok && scf_accumulate_launch(d_pos, d_mass, N, nmax, lmax, ws_scf, b0, b1 - b0, st) != cudaSuccess) fail();
+    }
+    if (ok && scf_finalize_launch(N, nmax, lmax, d_A, d_B, ws_scf, st) != cudaSuccess) fail();
+    if (ok && scf_force_launch(d_pos, N, nmax, lmax, d_A, d_B, ETICS_WHAT_BOTH, d_acc1, d_pot1, st) != cudaSuccess) fail();
+    link(st, cs);   // the SCF results go home while the MEX kernels run
+    copy(acc_scf_h, d_acc1, 3 * n * 8, cudaMemcpyDeviceToHost);
+    copy(pot_scf_h, d_pot1, n * 8, cudaMemcpyDeviceToHost);
+    if (A_h) copy(A_h, d_A, T * 8, cudaMemcpyDeviceToHost);
+    if (B_h) copy(B_h, d_B, T * 8, cudaMemcpyDeviceToHost);
+    if (ok && mex_force_launch(d_pos, d_mass, N, mex_lmax, ETICS_WHAT_BOTH, d_acc2, d_pot2, ws_mex, st) != cudaSuccess) fail();
+    (void)ws_mex_bytes;
+    link(st, cs);
+    copy(acc_mex_h, d_acc2, 3 * n * 8, cudaMemcpyDeviceToHost);
+    copy(pot_mex_h, d_pot2, n * 8, cudaMemcpyDeviceToHost);
+    link(cs, st);   // the caller's stream ends after the last copy
+    for (int i = 0; i < nev; ++i) cudaEventDestroy(ev[i]);
+    return ok ? ETICS_OK : ETICS_ERR_CUDA;
+}
+
 // ---- measurement support ---------------------------------------------------------------------------------
 etics_status etics_mex_force_timed(const double* pos, const double* mass, long long N, int lmax,
                                    double* acc, double* pot, void* workspace, size_t workspace_bytes, void* stream,

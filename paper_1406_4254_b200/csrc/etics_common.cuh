@@ -193,6 +193,10 @@ cudaError_t scf_init_constants();
 size_t scf_coeffs_workspace(long long N, int nmax, int lmax);
 cudaError_t scf_coeffs_launch(const double* pos, const double* mass, long long N, int nmax, int lmax,
                               double* A, double* B, void* ws, cudaStream_t st);
+int scf_coeffs_blocks(long long N, int nmax, int lmax, long long* particles_per_block);
+cudaError_t scf_accumulate_launch(const double* pos, const double* mass, long long N, int nmax, int lmax, void* ws,
+                                  int block0, int nblocks, cudaStream_t st);
+cudaError_t scf_finalize_launch(long long N, int nmax, int lmax, double* A, double* B, const void* ws, cudaStream_t st);
 cudaError_t scf_force_launch(const double* pos, long long N, int nmax, int lmax, const double* A, const double* B, int what,
                              double* acc, double* pot, cudaStream_t st);
 

@@ -243,6 +243,7 @@ struct AccGroup {
 struct AccPlan {
     int nmax, lmax, n1, L, T;
     int ngroups;
+    int block0;                // first block of this launch (the host entry launches ranges of blocks as their particles arrive)
     long long passes, passes_per_block;
     AccGroup group[kAccMaxGroups];
 };
@@ -363,7 +364,8 @@ scf_accumulate_kernel(const double* __restrict__ pos, const double* __restrict__
 #pragma unroll
         for (int j = 0; j < kAccWMax; ++j) acc[i][j] = 0.0;
 
-    const long long pass0 = (long long)blockIdx.x * pl.passes_per_block;
+    const int block = pl.block0 + (int)blockIdx.x;
+    const long long pass0 = (long long)block * pl.passes_per_block;
     const long long pass1 = min(pl.passes, pass0 + pl.passes_per_block);
 
     // raw coordinates of a pass: global -> shared with cp.async, thread k moves (and later reads) element k only
@@ -503,7 +505,7 @@ scf_accumulate_kernel(const double* __restrict__ pos, const double* __restrict__
         __syncthreads();
     }
     if (active && my_rep == 0 && lane == 0) {
-        double* out = partial + (size_t)blockIdx.x * 2 * pl.T;
+        double* out = partial + (size_t)block * 2 * pl.T;
 #pragma unroll
         for (int i = 0; i < kAccNCH; ++i)
 #pragma unroll
@@ -609,32 +611,50 @@ size_t scf_coeffs_workspace(long long N, int nmax, int lmax) {
 }
 
 template <int LMAX>
-static cudaError_t launch_accumulate(const double* pos, const double* mass, long long N, const AccPlan& p, int bx,
+static cudaError_t launch_accumulate(const double* pos, const double* mass, long long N, const AccPlan& p, int nblocks,
                                      double* partial, cudaStream_t st) {
     const size_t smem = acc_smem_bytes(p);
-    if (p.ngroups == 1) scf_accumulate_kernel<LMAX, true><<<dim3(bx, 1), kAccThreads, smem, st>>>(pos, mass, N, p, partial);
-    else scf_accumulate_kernel<LMAX, false><<<dim3(bx, p.ngroups), kAccThreads, smem, st>>>(pos, mass, N, p, partial);
+    if (p.ngroups == 1) scf_accumulate_kernel<LMAX, true><<<dim3(nblocks, 1), kAccThreads, smem, st>>>(pos, mass, N, p, partial);
+    else scf_accumulate_kernel<LMAX, false><<<dim3(nblocks, p.ngroups), kAccThreads, smem, st>>>(pos, mass, N, p, partial);
     return cudaGetLastError();
 }
 
-cudaError_t scf_coeffs_launch(const double* pos, const double* mass, long long N, int nmax, int lmax,
-                              double* A, double* B, void* ws, cudaStream_t st) {
+// Blocks of the accumulation and the particles [first, last) block b works on: the host entry point uploads and
+// accumulates ranges of whole blocks, which leaves every block partial — and so A, B — bit-identical to one launch.
+int scf_coeffs_blocks(long long N, int nmax, int lmax, long long* particles_per_block) {
+    const AccPlan p = make_acc_plan(N, nmax, lmax);
+    if (particles_per_block) *particles_per_block = p.passes_per_block * kAccP;
+    return acc_blocks_x(p);
+}
+
+cudaError_t scf_accumulate_launch(const double* pos, const double* mass, long long N, int nmax, int lmax, void* ws,
+                                  int block0, int nblocks, cudaStream_t st) {
     cudaError_t e = scf_init_constants();
     if (e != cudaSuccess) return e;
-    const AccPlan p = make_acc_plan(N, nmax, lmax);
+    AccPlan p = make_acc_plan(N, nmax, lmax);
+    p.block0 = block0;
     double* partial = static_cast<double*>(ws);
-    const int bx = acc_blocks_x(p);
     switch (lmax) {
-#define ETICS_CASE(LM) case LM: e = launch_accumulate<LM>(pos, mass, N, p, bx, partial, st); break;
+#define ETICS_CASE(LM) case LM: return launch_accumulate<LM>(pos, mass, N, p, nblocks, partial, st);
         ETICS_CASE(0) ETICS_CASE(1) ETICS_CASE(2) ETICS_CASE(3) ETICS_CASE(4) ETICS_CASE(5)
         ETICS_CASE(6) ETICS_CASE(7) ETICS_CASE(8) ETICS_CASE(9) ETICS_CASE(10)
 #undef ETICS_CASE
         default: return cudaErrorInvalidValue;
     }
-    if (e != cudaSuccess) return e;
+}
+
+cudaError_t scf_finalize_launch(long long N, int nmax, int lmax, double* A, double* B, const void* ws, cudaStream_t st) {
+    const AccPlan p = make_acc_plan(N, nmax, lmax);
     const int T2 = 2 * p.T, wpb = kFinThreads / 32;
-    scf_finalize_kernel<<<(T2 + wpb - 1) / wpb, kFinThreads, 0, st>>>(partial, bx, nmax, lmax, A, B);
+    scf_finalize_kernel<<<(T2 + wpb - 1) / wpb, kFinThreads, 0, st>>>(static_cast<const double*>(ws), acc_blocks_x(p), nmax, lmax, A, B);
     return cudaGetLastError();
+}
+
+cudaError_t scf_coeffs_launch(const double* pos, const double* mass, long long N, int nmax, int lmax,
+                              double* A, double* B, void* ws, cudaStream_t st) {
+    cudaError_t e = scf_accumulate_launch(pos, mass, N, nmax, lmax, ws, 0, scf_coeffs_blocks(N, nmax, lmax, nullptr), st);
+    if (e != cudaSuccess) return e;
+    return scf_finalize_launch(N, nmax, lmax, A, B, ws, st);
 }
 
 // nmax = 10 (the paper's cut-off) at lmax <= 6 gets fully unrolled n loops: 166.5 -> 149 us at N = 1e6.

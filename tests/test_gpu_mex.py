@@ -248,3 +248,35 @@ def test_force_only_and_potential_only(E, lmax):
     assert rel_err_scalar(pot_p.cpu().numpy(), pot.cpu().numpy(), floor=0.0) <= 1e-14
     assert E.lib().etics_mex_force_ex(dpos.data_ptr(), dmass.data_ptr(), pos.shape[1], lmax, 7,
                                       acc.data_ptr(), pot.data_ptr(), ws.data_ptr(), ws.numel(), st) == E.ETICS_ERR_ARG
+
+
+@pytest.mark.parametrize("two_streams", [False, True])
+@pytest.mark.parametrize("n", [30_000, 400_003])
+def test_step_host_entry_point(E, n, two_streams):
+    """etics_step_host: one upload, both methods, overlapped copies — against the oracle, and bit-identical to the
+    device-pointer calls (the upload is accumulated in ranges of whole blocks, so every block partial is unchanged)."""
+    pos, mass = W.particles("hernquist", n, seed=3, axes=(1.0, 0.9, 0.8))
+    pos_h, mass_h = torch.from_numpy(pos).pin_memory(), torch.from_numpy(mass).pin_memory()
+    out = [torch.empty((3, n), dtype=torch.float64).pin_memory(), torch.empty(n, dtype=torch.float64).pin_memory(),
+           torch.empty((3, n), dtype=torch.float64).pin_memory(), torch.empty(n, dtype=torch.float64).pin_memory()]
+    T = 11 * E.num_lm(6)
+    A_h, B_h = torch.empty(T, dtype=torch.float64).pin_memory(), torch.empty(T, dtype=torch.float64).pin_memory()
+    scratch = torch.empty(E.etics_step_host_scratch_bytes(n, 10, 6, 4), dtype=torch.uint8, device="cuda")
+    cs = torch.cuda.Stream() if two_streams else None
+    for _ in range(2):   # a second call reuses the scratch while nothing is in flight
+        E.etics_step_host(pos_h, mass_h, 10, 6, 4, out[0], out[1], out[2], out[3], scratch, A_h, B_h, copy_stream=cs)
+        torch.cuda.current_stream().synchronize()
+    dpos, dmass = dev(pos), dev(mass)
+    A, B = E.etics_scf_coeffs(dpos, dmass, 10, 6)
+    acc1, pot1 = E.etics_scf_force(dpos, 10, 6, A, B)
+    acc2, pot2 = E.etics_mex_force(dpos, dmass, 4)
+    torch.cuda.synchronize()
+    for h, d in zip([A_h, B_h] + out, [A, B, acc1, pot1, acc2, pot2]):
+        assert np.array_equal(h.numpy(), d.cpu().numpy())
+    if n <= 30_000:
+        A0, B0 = oracle.scf_coeffs(pos, mass, 10, 6)
+        acc0, pot0 = oracle.scf_force(pos, 10, 6, A0, B0)
+        assert rel_err_scalar(A_h.numpy(), A0) <= TOL and rel_err_vector(out[0].numpy(), acc0) <= TOL
+        assert rel_err_scalar(out[1].numpy(), pot0, floor=0.0) <= TOL
+        accm, potm = oracle.mex_force(pos, mass, 4)
+        assert rel_err_vector(out[2].numpy(), accm) <= TOL and rel_err_scalar(out[3].numpy(), potm, floor=0.0) <= TOL
