@@ -25,7 +25,7 @@ EXPORTS = [
     "etics_status_string", "etics_init", "etics_workspace_bytes", "etics_scf_coeffs", "etics_scf_force",
     "etics_mex_force", "etics_scf_force_ex", "etics_mex_force_ex", "etics_mex_sort", "etics_host_scratch_bytes", "etics_scf_full_host",
     "etics_mex_full_host", "etics_mex_force_timed", "etics_probe_dfma", "etics_probe_copy",
-    "etics_step_host_scratch_bytes", "etics_step_host", "etics_stepper_workspace_bytes", "etics_stepper_create", "etics_stepper_step", "etics_stepper_destroy",
+    "etics_kernel_launches", "etics_step_host_scratch_bytes", "etics_step_host", "etics_stepper_workspace_bytes", "etics_stepper_create", "etics_stepper_step", "etics_stepper_destroy",
 ]
 
 _lib = None
@@ -74,6 +74,8 @@ def lib() -> C.CDLL:
     L.etics_mex_full_host.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _vp, _sz, _vp]
     L.etics_mex_force_timed.restype = _i
     L.etics_mex_force_timed.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _vp, _sz, _vp, C.POINTER(C.c_float)]
+    L.etics_kernel_launches.restype = _i
+    L.etics_kernel_launches.argtypes = [_i, _ll]
     L.etics_step_host_scratch_bytes.restype = _sz
     L.etics_step_host_scratch_bytes.argtypes = [_ll, _i, _i, _i]
     L.etics_step_host.restype = _i
@@ -264,6 +266,10 @@ def etics_mex_full_host(pos_h, mass_h, lmax: int, acc_h, pot_h, scratch, stream=
                                   _host(acc_h, "acc_h"), _host(pot_h, "pot_h"),
                                   scratch.data_ptr(), scratch.numel() * scratch.element_size(), _stream(stream))
     _check(s, "etics_mex_full_host")
+
+
+def etics_kernel_launches(which: int, N: int) -> int:
+    return lib().etics_kernel_launches(which, N)
 
 
 def etics_step_host_scratch_bytes(N: int, nmax: int, lmax: int, mex_lmax: int) -> int:

@@ -276,6 +276,15 @@ etics_status etics_mex_force_timed(const double* pos, const double* mass, long l
     return from_cuda(mex_force_timed(pos, mass, N, lmax, acc, pot, workspace, static_cast<cudaStream_t>(stream), stage_ms));
 }
 
+int etics_kernel_launches(int which, long long N) {
+    switch (which) {
+        case ETICS_WS_SCF_COEFFS: return 2;
+        case ETICS_WS_SCF_FORCE: return 1;
+        case ETICS_WS_MEX_FORCE: return (N >= 1 && N < (1LL << 31)) ? mex_kernel_launches(N) : 0;
+        default: return 0;
+    }
+}
+
 // ---- probes ----------------------------------------------------------------------------------------------
 etics_status etics_probe_dfma(int iters, double* sink, double* flops_out, void* stream) {
     if (iters < 1 || !sink) return ETICS_ERR_ARG;

@@ -201,6 +201,7 @@ cudaError_t scf_force_launch(const double* pos, long long N, int nmax, int lmax,
                              double* acc, double* pot, cudaStream_t st);
 
 cudaError_t mex_init_constants();
+int mex_kernel_launches(long long N);
 size_t mex_workspace(long long N, int lmax);
 cudaError_t mex_sort_launch(const double* pos, long long N, unsigned long long* keys_sorted, unsigned int* perm,
                             void* ws, cudaStream_t st);

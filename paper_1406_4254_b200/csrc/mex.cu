@@ -37,6 +37,7 @@
 namespace etics {
 
 #if ETICS_MEX_PART == 0
+int mex_kernel_launches(long long N) { return mex_sort_kernel_launches(N) + 4; }   // + gather/totals, tile scan, evaluate, unpack
 cudaError_t mex_init_constants() { return mex_sort_init_device(); }   // every MEX constant is a compile-time literal; per-device function attributes
 #endif
 

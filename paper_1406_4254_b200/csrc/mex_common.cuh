@@ -62,5 +62,6 @@ cudaError_t mex_sort_enqueue(const double* pos, const double* mass, long long N,
                              unsigned* perm_out, unsigned long long* keys_sorted_out, bool pack, cudaStream_t st,
                              cudaEvent_t ev_keygen);
 cudaError_t mex_sort_init_device();
+int mex_sort_kernel_launches(long long N);
 
 }  // namespace etics

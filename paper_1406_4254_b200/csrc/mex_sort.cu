@@ -815,6 +815,15 @@ static cudaError_t sort_device(SortDevice* out) {
     return cudaSuccess;
 }
 
+// kernels one sort launches (for the launch count bench.py reports): the cooperative kernel + the fallback kernel, or
+// keys + (histogram, scan, scatter) per pass + the two fix-up kernels + the fallback kernel
+int mex_sort_kernel_launches(long long N) {
+    SortDevice dv;
+    if (sort_device(&dv) != cudaSuccess) return 0;
+    const long long tiles = (N + kSortTile - 1) / kSortTile;
+    return tiles <= dv.small_blocks ? 2 : 1 + 3 * (kLargePrefixBits / kLargeDB) + 2 + 1;
+}
+
 cudaError_t mex_sort_init_device() {
     SortDevice d;
     return sort_device(&d);
