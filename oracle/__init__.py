@@ -170,11 +170,18 @@ def leapfrog(force, pos, vel, dt: float, nsteps: int):
     return x, v, a
 
 
-def scf_acceleration(mass, nmax: int, lmax: int):
-    """force(pos) for leapfrog(): the SCF full force calculation on the particles themselves."""
+def scf_acceleration(mass, nmax: int, lmax: int, every: int = 1):
+    """force(pos) for leapfrog(): the SCF full force calculation on the particles themselves.  every > 1: "temporal
+    softening": the coefficients are recomputed at force evaluations 0, every, 2 every, ... and held in
+    between (evaluation 0 is a(x_0), evaluation j the force of step j)."""
+    state = {"calls": 0, "AB": None}
+
     def f(x):
-        A, B = scf_coeffs(x, mass, nmax, lmax)
-        return scf_force(x, nmax, lmax, A, B)[0]
+        if state["calls"] % every == 0:
+            state["AB"] = scf_coeffs(x, mass, nmax, lmax)
+        state["calls"] += 1
+        return scf_force(x, nmax, lmax, *state["AB"])[0]
+    f.state = state
     return f
 
 

@@ -25,7 +25,7 @@ EXPORTS = [
     "etics_status_string", "etics_init", "etics_workspace_bytes", "etics_scf_coeffs", "etics_scf_force",
     "etics_mex_force", "etics_scf_force_ex", "etics_mex_force_ex", "etics_mex_sort", "etics_host_scratch_bytes", "etics_scf_full_host",
     "etics_mex_full_host", "etics_mex_force_timed", "etics_probe_dfma", "etics_probe_copy",
-    "etics_kernel_launches", "etics_step_host_scratch_bytes", "etics_step_host", "etics_stepper_workspace_bytes", "etics_stepper_create", "etics_stepper_step", "etics_stepper_destroy",
+    "etics_kernel_launches", "etics_step_host_scratch_bytes", "etics_step_host", "etics_stepper_workspace_bytes", "etics_stepper_create", "etics_stepper_step", "etics_stepper_set_coefficient_interval", "etics_stepper_destroy",
 ]
 
 _lib = None
@@ -86,6 +86,8 @@ def lib() -> C.CDLL:
     L.etics_stepper_create.argtypes = [C.POINTER(_vp), _i, _vp, _vp, _vp, _ll, _i, _i, C.c_double, _vp, _vp, _vp, _sz, _i, _vp]
     L.etics_stepper_step.restype = _i
     L.etics_stepper_step.argtypes = [_vp, _i]
+    L.etics_stepper_set_coefficient_interval.restype = _i
+    L.etics_stepper_set_coefficient_interval.argtypes = [_vp, _i]
     L.etics_stepper_destroy.restype = _i
     L.etics_stepper_destroy.argtypes = [_vp]
     L.etics_probe_dfma.restype = _i
@@ -319,6 +321,9 @@ class Stepper:
                                        self.workspace.numel(), int(bool(use_graph)), _stream(stream))
         _check(s, "etics_stepper_create")
         self._h = h
+
+    def set_coefficient_interval(self, every: int) -> None:
+        _check(lib().etics_stepper_set_coefficient_interval(self._h, every), "etics_stepper_set_coefficient_interval")
 
     def step(self, nsteps: int = 1) -> None:
         _check(lib().etics_stepper_step(self._h, nsteps), "etics_stepper_step")

@@ -46,8 +46,10 @@ cudaError_t mex_init_constants() { return mex_sort_init_device(); }   // every M
 // =========================================================================================================
 // Column -> group tables: greedy balanced partition (columns in descending count of running sums, each to the least
 // loaded group) for a target of 28 running sums per direction and group; generated offline, fixed at compile time.
-// (Targets of 18 and 13 — 126 registers/thread, 16 resident warps per SM instead of 12 — were measured: no gain.)
+// (Targets of 17 and 13 sums per group — 3 and 4 groups at lmax 6, 128 registers, 16 resident warps per SM instead of 12 —
+// were measured again with the fused kernel: 125 -> 139 and 154 us at N = 1e6: every group repeats the per-particle set-up.)
 constexpr int kMexMaxGroups = 8;
+
 #define ETICS_MEX_NG_INIT {1, 1, 1, 1, 1, 2, 2, 3, 3, 4, 5}
 #define ETICS_MEX_GOF_INIT { \
     {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, \
@@ -189,11 +191,13 @@ struct Angles {
     double cm[LMAX + 1], sm[LMAX + 1];   // cos m phi, sin m phi
     double sp1[LMAX + 1];                // st^(m-1), m >= 1
     __device__ __forceinline__ void init(const Rec& p) {
+        // cos(m phi), sin(m phi) by the three-term recurrence f_m = 2 cos(phi) f_{m-1} - f_{m-2}: one FMA per value
         cm[0] = 1.0; sm[0] = 0.0; sp1[0] = 0.0;
+        const double tc = p.cp + p.cp;
 #pragma unroll
         for (int m = 1; m <= LMAX; ++m) {
-            cm[m] = fma(cm[m - 1], p.cp, -sm[m - 1] * p.sp);
-            sm[m] = fma(sm[m - 1], p.cp, cm[m - 1] * p.sp);
+            cm[m] = (m == 1) ? p.cp : fma(tc, cm[m - 1], -cm[m - 2]);
+            sm[m] = (m == 1) ? p.sp : fma(tc, sm[m - 1], -sm[m - 2]);
             sp1[m] = (m == 1) ? 1.0 : sp1[m - 1] * p.st;
         }
     }

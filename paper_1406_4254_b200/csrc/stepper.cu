@@ -45,30 +45,34 @@ struct etics_stepper {
     void* ws;               // force workspace
     size_t ws_bytes;
     cudaStream_t stream;
-    cudaGraph_t graph;
-    cudaGraphExec_t exec;
+    cudaGraph_t graph[2];       // [0] step with fresh coefficients, [1] step with the held coefficients (SCF only)
+    cudaGraphExec_t exec[2];
     bool have_acc;          // acc holds a(pos)
+    int every;              // SCF: coefficients are recomputed at force evaluations 0, every, 2 every, ... (temporal softening)
+    long long evals;        // force evaluations so far
 };
 
 namespace {
 
 size_t stepper_table_bytes(int nmax, int lmax) { return round_up((size_t)(nmax + 1) * num_lm(lmax) * sizeof(double), 256); }
 
-etics_status stepper_force(etics_stepper* s) {
+etics_status stepper_force(etics_stepper* s, bool fresh) {
     if (s->method == 0) {
-        etics_status e = etics_scf_coeffs(s->pos, s->mass, s->N, s->nmax, s->lmax, s->A, s->B, s->ws, s->ws_bytes, s->stream);
-        if (e != ETICS_OK) return e;
+        if (fresh) {
+            const etics_status e = etics_scf_coeffs(s->pos, s->mass, s->N, s->nmax, s->lmax, s->A, s->B, s->ws, s->ws_bytes, s->stream);
+            if (e != ETICS_OK) return e;
+        }
         return etics_scf_force(s->pos, s->N, s->nmax, s->lmax, s->A, s->B, s->acc, s->pot, nullptr, 0, s->stream);
     }
     return etics_mex_force(s->pos, s->mass, s->N, s->lmax, s->acc, s->pot, s->ws, s->ws_bytes, s->stream);
 }
 
-etics_status stepper_enqueue_step(etics_stepper* s) {
+etics_status stepper_enqueue_step(etics_stepper* s, bool fresh) {
     const long long n3 = 3 * s->N;
     const unsigned blocks = (unsigned)((n3 + 255) / 256);
     leapfrog_kick_drift_kernel<<<blocks, 256, 0, s->stream>>>(s->pos, s->vel, s->acc, n3, 0.5 * s->dt, s->dt);
     if (cudaGetLastError() != cudaSuccess) return ETICS_ERR_CUDA;
-    etics_status e = stepper_force(s);
+    etics_status e = stepper_force(s, fresh);
     if (e != ETICS_OK) return e;
     leapfrog_kick_kernel<<<blocks, 256, 0, s->stream>>>(s->vel, s->acc, n3, 0.5 * s->dt);
     return cudaGetLastError() == cudaSuccess ? ETICS_OK : ETICS_ERR_CUDA;
@@ -116,41 +120,59 @@ etics_status etics_stepper_create(etics_stepper** out, int method, double* pos, 
         s->ws_bytes = workspace_bytes;
     }
     s->ws = w;
+    s->every = 1;
     if (use_graph) {
         // the step's launch sequence is recorded once; replaying it costs one launch per step instead of 4-17.  It is
         // recorded on a stream of its own (capturing work is not executed, and the caller's stream may be the legacy
         // default stream, which cannot capture); the graph is then launched on the caller's stream.
         cudaStream_t cap = nullptr, user = s->stream;
         if (cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) != cudaSuccess) { delete s; return ETICS_ERR_CUDA; }
-        etics_status e = ETICS_ERR_CUDA;
-        cudaGraph_t g = nullptr;
-        if (cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-            s->stream = cap;
-            e = stepper_enqueue_step(s);
-            s->stream = user;
-            if (cudaStreamEndCapture(cap, &g) != cudaSuccess && e == ETICS_OK) e = ETICS_ERR_CUDA;
+        etics_status e = ETICS_OK;
+        for (int v = 0; v < (method == 0 ? 2 : 1) && e == ETICS_OK; ++v) {
+            e = ETICS_ERR_CUDA;
+            cudaGraph_t g = nullptr;
+            if (cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                s->stream = cap;
+                e = stepper_enqueue_step(s, v == 0);
+                s->stream = user;
+                if (cudaStreamEndCapture(cap, &g) != cudaSuccess && e == ETICS_OK) e = ETICS_ERR_CUDA;
+            }
+            s->graph[v] = g;
+            if (e == ETICS_OK && (!g || cudaGraphInstantiate(&s->exec[v], g, 0) != cudaSuccess)) e = ETICS_ERR_CUDA;
         }
         cudaStreamDestroy(cap);
-        if (e == ETICS_OK && (!g || cudaGraphInstantiate(&s->exec, g, 0) != cudaSuccess)) e = ETICS_ERR_CUDA;
-        if (e != ETICS_OK) { if (g) cudaGraphDestroy(g); delete s; cudaGetLastError(); return e; }
-        s->graph = g;
+        if (e != ETICS_OK) {
+            for (int v = 0; v < 2; ++v) { if (s->exec[v]) cudaGraphExecDestroy(s->exec[v]); if (s->graph[v]) cudaGraphDestroy(s->graph[v]); }
+            delete s;
+            cudaGetLastError();
+            return e;
+        }
     }
     *out = s;
     return ETICS_OK;
 }
 
+etics_status etics_stepper_set_coefficient_interval(etics_stepper* s, int every) {
+    if (!s || every < 1 || s->method != 0 || s->have_acc) return ETICS_ERR_ARG;
+    s->every = every;
+    return ETICS_OK;
+}
+
 etics_status etics_stepper_step(etics_stepper* s, int nsteps) {
     if (!s || nsteps < 0) return ETICS_ERR_ARG;
-    if (!s->have_acc) {   // a(x_0)
-        const etics_status e = stepper_force(s);
+    if (!s->have_acc) {   // a(x_0): force evaluation 0
+        const etics_status e = stepper_force(s, true);
         if (e != ETICS_OK) return e;
         s->have_acc = true;
+        s->evals = 1;
     }
-    for (int i = 0; i < nsteps; ++i) {
-        if (s->exec) {
-            if (cudaGraphLaunch(s->exec, s->stream) != cudaSuccess) return ETICS_ERR_CUDA;
+    for (int i = 0; i < nsteps; ++i, ++s->evals) {
+        const bool fresh = s->method != 0 || s->evals % s->every == 0;
+        cudaGraphExec_t g = s->exec[fresh ? 0 : 1];
+        if (g) {
+            if (cudaGraphLaunch(g, s->stream) != cudaSuccess) return ETICS_ERR_CUDA;
         } else {
-            const etics_status e = stepper_enqueue_step(s);
+            const etics_status e = stepper_enqueue_step(s, fresh);
             if (e != ETICS_OK) return e;
         }
     }
@@ -160,11 +182,11 @@ etics_status etics_stepper_step(etics_stepper* s, int nsteps) {
 etics_status etics_stepper_destroy(etics_stepper* s) {
     if (!s) return ETICS_OK;
     cudaError_t e = cudaSuccess;
-    if (s->exec) {
-        e = cudaStreamSynchronize(s->stream);   // the graph must not be in flight when it is destroyed
-        cudaGraphExecDestroy(s->exec);
+    if (s->exec[0]) e = cudaStreamSynchronize(s->stream);   // a graph must not be in flight when it is destroyed
+    for (int v = 0; v < 2; ++v) {
+        if (s->exec[v]) cudaGraphExecDestroy(s->exec[v]);
+        if (s->graph[v]) cudaGraphDestroy(s->graph[v]);
     }
-    if (s->graph) cudaGraphDestroy(s->graph);
     delete s;
     return e == cudaSuccess ? ETICS_OK : ETICS_ERR_CUDA;
 }

@@ -97,3 +97,19 @@ def test_stepper_argument_errors(E):
     assert h.value is None
     assert E.lib().etics_stepper_step(None, 1) == E.ETICS_ERR_ARG
     assert E.lib().etics_stepper_destroy(None) == E.ETICS_OK
+
+
+@pytest.mark.parametrize("graph", [False, True])
+def test_scf_temporal_softening(E, graph):
+    """coefficients refreshed every 4th force evaluation, held in between."""
+    n, dt, nsteps, nmax, lmax, every = 2_000, 0.01, 10, 8, 5, 4
+    pos, vel, mass = initial_conditions(n, 14)
+    dpos, dvel, dmass = (torch.from_numpy(a.copy()).cuda() for a in (pos, vel, mass))
+    s = E.Stepper(0, dpos, dvel, dmass, dt, nmax=nmax, lmax=lmax, use_graph=graph)
+    s.set_coefficient_interval(every)
+    s.step(3); s.step(nsteps - 3)
+    torch.cuda.synchronize()
+    x0, v0, a0 = oracle.leapfrog(oracle.scf_acceleration(mass, nmax, lmax, every=every), pos, vel, dt, nsteps)
+    check(dpos.cpu().numpy(), dvel.cpu().numpy(), s.acc.cpu().numpy(), x0, v0, a0, nsteps * dt)
+    assert E.lib().etics_stepper_set_coefficient_interval(s._h, 2) == E.ETICS_ERR_ARG   # only before the first step
+    s.close()

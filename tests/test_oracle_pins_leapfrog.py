@@ -75,3 +75,32 @@ def test_mex_leapfrog_energy_and_two_body_radial_fall():
     E1 = 0.5 * v[0, 1] ** 2 - 1.0 / x[0, 1]
     assert x[0, 1] < 2.0 and v[0, 1] < 0.0 and abs(E1 - E0) < 1e-6
     assert np.all(x[1:, 1] == 0.0)
+
+
+def test_temporal_softening_static_field_conserves_particle_energies():
+    # coefficients held over many steps = motion in a STATIC potential, in which the energy of every particle,
+    # v^2/2 + Phi(x) with Phi from the held coefficients, is conserved by the leapfrog to O(dt^2); with every = 1 the helper
+    # is the plain force.  (A wrong refresh schedule moves the potential under the particles and breaks the first part;
+    # a stale acceleration breaks the second.)
+    from paper_1406_4254_b200 import workloads as W
+    pos, mass = W.particles("hernquist", 400, seed=21)
+    vel = 0.3 * np.stack([W.uniforms(21, 400, 3 + k) - 0.5 for k in range(3)])
+    f = oracle.scf_acceleration(mass, 6, 4, every=10_000)
+    x, v, _ = oracle.leapfrog(f, pos, vel, 0.002, 50)
+    A, B = f.state["AB"]
+    assert f.state["calls"] == 51
+    A0, B0 = oracle.scf_coeffs(pos, mass, 6, 4)
+    assert np.array_equal(A, A0) and np.array_equal(B, B0)          # still the coefficients of x_0
+    E0 = 0.5 * np.sum(vel ** 2, axis=0) + oracle.scf_force(pos, 6, 4, A, B)[1]
+    E1 = 0.5 * np.sum(v ** 2, axis=0) + oracle.scf_force(x, 6, 4, A, B)[1]
+    assert np.max(np.abs(E1 - E0) / np.abs(E0)) < 2e-4
+    x1, v1, _ = oracle.leapfrog(oracle.scf_acceleration(mass, 6, 4, every=1), pos, vel, 0.002, 5)
+    x2, v2, _ = oracle.leapfrog(oracle.scf_acceleration(mass, 6, 4), pos, vel, 0.002, 5)
+    assert np.array_equal(x1, x2) and np.array_equal(v1, v2)
+    # the schedule: every = 3 refreshes at evaluations 0, 3, 6 -> after 7 steps the held table belongs to x_6
+    f3 = oracle.scf_acceleration(mass, 6, 4, every=3)
+    xs = []
+    g = lambda xx: (xs.append(xx.copy()), f3(xx))[1]
+    oracle.leapfrog(g, pos, vel, 0.002, 7)
+    A6, _ = oracle.scf_coeffs(xs[6], mass, 6, 4)
+    assert np.array_equal(f3.state["AB"][0], A6)
