@@ -305,32 +305,55 @@ def etics_probe_copy(dst, src, stream=None) -> int:
     return 2 * nbytes
 
 
+def etics_stepper_workspace_bytes(method: int, N: int, nmax: int, lmax: int) -> int:
+    return lib().etics_stepper_workspace_bytes(method, N, nmax, lmax)
+
+
+def etics_stepper_create(method: int, pos, vel, mass, nmax: int, lmax: int, dt: float, acc, pot, workspace, use_graph: bool = True,
+                         stream=None):
+    """Returns the opaque handle (a ctypes void pointer) of a stepper over the caller's CUDA tensors."""
+    h = _vp()
+    s = lib().etics_stepper_create(C.byref(h), method, _dev(pos, "pos"), _dev(vel, "vel"), _dev(mass, "mass"), mass.shape[0], nmax, lmax,
+                                   float(dt), _dev(acc, "acc"), _dev(pot, "pot"), workspace.data_ptr(),
+                                   workspace.numel() * workspace.element_size(), int(bool(use_graph)), _stream(stream))
+    _check(s, "etics_stepper_create")
+    return h
+
+
+def etics_stepper_step(handle, nsteps: int = 1) -> None:
+    _check(lib().etics_stepper_step(handle, nsteps), "etics_stepper_step")
+
+
+def etics_stepper_set_coefficient_interval(handle, every: int) -> None:
+    _check(lib().etics_stepper_set_coefficient_interval(handle, every), "etics_stepper_set_coefficient_interval")
+
+
+def etics_stepper_destroy(handle) -> None:
+    _check(lib().etics_stepper_destroy(handle), "etics_stepper_destroy")
+
+
 class Stepper:
-    """Handle of etics_stepper_* (include/etics.h): kick-drift-kick steps with the SCF (method 0) or MEX (method 1) force.
-    pos, vel are updated in place; acc, pot hold the acceleration / potential at the current positions."""
+    """Keeps the tensors a stepper handle refers to alive (etics_stepper_* of include/etics.h): kick-drift-kick steps with
+    the SCF (method 0) or MEX (method 1) force.  pos, vel are updated in place; acc, pot hold the acceleration / potential
+    at the current positions."""
 
     def __init__(self, method: int, pos, vel, mass, dt: float, nmax: int = 0, lmax: int = 0, use_graph: bool = True, stream=None):
         N = mass.shape[0]
         self.pos, self.vel, self.mass = pos, vel, mass
         self.acc = torch.empty((3, N), dtype=torch.float64, device=pos.device)
         self.pot = torch.empty(N, dtype=torch.float64, device=pos.device)
-        self.workspace = torch.empty(lib().etics_stepper_workspace_bytes(method, N, nmax, lmax), dtype=torch.uint8, device=pos.device)
-        h = _vp()
-        s = lib().etics_stepper_create(C.byref(h), method, _dev(pos, "pos"), _dev(vel, "vel"), _dev(mass, "mass"), N, nmax, lmax,
-                                       float(dt), _dev(self.acc, "acc"), _dev(self.pot, "pot"), self.workspace.data_ptr(),
-                                       self.workspace.numel(), int(bool(use_graph)), _stream(stream))
-        _check(s, "etics_stepper_create")
-        self._h = h
+        self.workspace = torch.empty(etics_stepper_workspace_bytes(method, N, nmax, lmax), dtype=torch.uint8, device=pos.device)
+        self._h = etics_stepper_create(method, pos, vel, mass, nmax, lmax, dt, self.acc, self.pot, self.workspace, use_graph, stream)
 
     def set_coefficient_interval(self, every: int) -> None:
-        _check(lib().etics_stepper_set_coefficient_interval(self._h, every), "etics_stepper_set_coefficient_interval")
+        etics_stepper_set_coefficient_interval(self._h, every)
 
     def step(self, nsteps: int = 1) -> None:
-        _check(lib().etics_stepper_step(self._h, nsteps), "etics_stepper_step")
+        etics_stepper_step(self._h, nsteps)
 
     def close(self) -> None:
         if self._h is not None:
-            _check(lib().etics_stepper_destroy(self._h), "etics_stepper_destroy")
+            etics_stepper_destroy(self._h)
             self._h = None
 
     def __del__(self):
