@@ -101,6 +101,7 @@ struct SortParams {
     unsigned* seg_hist;       // [nseg][kSortBins]
     unsigned* bin_tot;        // [kSortBins]
     unsigned* perm;
+    unsigned* itmp;           // second index buffer of the fallback sort
     unsigned long long* keys_sorted;   // may be null
     long long tiles, tps;     // tiles of kSortTile words; tiles per segment
     int nseg;
@@ -606,6 +607,86 @@ __device__ __forceinline__ void sort_phase_fixruns(const SortParams& P, const So
     }
 }
 
+// =========================================================================================================
+// Fallback: stable LSD sort of (full key, index), eight 8-bit passes, ONE block (histogram by all threads, stable
+// scatter by warp 0, 32 keys per step).  Runs only when the fix-up raised the flag.
+// =========================================================================================================
+__device__ __noinline__ void sort_fallback_block(const unsigned long long* keys, long long N,
+                                                 unsigned long long* kA, unsigned long long* kB, unsigned* iA, unsigned* iB,
+                                                 unsigned long long* keys_sorted) {
+    __shared__ unsigned hist[256];
+    __shared__ unsigned base[256];
+    __shared__ int single;
+    const int nthr = blockDim.x;   // >= 256
+    const int tid = threadIdx.x, lane = tid & 31;
+    int cur = -1;   // -1: the source is (keys, identity); 0: set A; 1: set B
+    for (int pass = 0; pass < 8; ++pass) {
+        const int shift = 8 * pass;
+        const unsigned long long* ksrc = (cur < 0) ? keys : (cur == 0 ? kA : kB);
+        const unsigned* isrc = (cur < 0) ? nullptr : (cur == 0 ? iA : iB);
+        unsigned long long* kdst = (cur == 0) ? kB : kA;
+        unsigned* idst = (cur == 0) ? iB : iA;
+        if (tid < 256) hist[tid] = 0;
+        if (tid == 0) single = 0;
+        __syncthreads();
+        for (long long k = tid; k < N; k += nthr) atomicAdd(&hist[(unsigned)(ksrc[k] >> shift) & 255u], 1u);
+        __syncthreads();
+        if (tid < 256 && hist[tid] == (unsigned)N) single = 1;
+        __syncthreads();
+        const bool skip = single != 0 && cur >= 0;   // every key has the same digit: a stable pass would change nothing
+        __syncthreads();                              // `single` is rewritten at the top of the next pass
+        if (skip) continue;
+        if (tid == 0) {
+            unsigned run = 0;
+            for (int d = 0; d < 256; ++d) { base[d] = run; run += hist[d]; }
+        }
+        __syncthreads();
+        if (tid < 32) {
+            for (long long k0 = 0; k0 < N; k0 += 32) {
+                const long long k = k0 + lane;
+                const bool ok = k < N;
+                const unsigned long long key = ok ? ksrc[k] : 0ull;
+                const unsigned d = ok ? ((unsigned)(key >> shift) & 255u) : 256u;
+                unsigned peers = 0xffffffffu;
+#pragma unroll
+                for (int b = 0; b < 9; ++b) {
+                    const bool bit = (d >> b) & 1u;
+                    const unsigned vote = __ballot_sync(0xffffffffu, bit);
+                    peers &= bit ? vote : ~vote;
+                }
+                if (ok) {
+                    const unsigned lower = peers & ((1u << lane) - 1u);
+                    const unsigned g = base[d] + __popc(lower);
+                    kdst[g] = key;
+                    idst[g] = isrc ? isrc[k] : (unsigned)k;
+                }
+                __syncwarp();
+                if (ok && (peers & ((1u << lane) - 1u)) == 0u) base[d] += __popc(peers);
+                __syncwarp();
+            }
+        }
+        __threadfence();
+        __syncthreads();
+        cur = (cur == 0) ? 1 : 0;
+    }
+    // the result belongs in set A (iA is the caller's permutation)
+    if (cur == 1) {
+        for (long long k = tid; k < N; k += nthr) { kA[k] = kB[k]; iA[k] = iB[k]; }
+        __threadfence();
+        __syncthreads();
+    }
+    if (keys_sorted)
+        for (long long k = tid; k < N; k += nthr) keys_sorted[k] = kA[k];
+}
+
+__global__ void __launch_bounds__(1024)
+mex_sort_fallback_kernel(const SortHeader* __restrict__ hdr, const unsigned long long* keys, long long N,
+                         unsigned long long* kA, unsigned long long* kB, unsigned* iA, unsigned* iB,
+                         unsigned long long* keys_sorted) {
+    if (__ldcg(&hdr->fallback) == 0u) return;
+    sort_fallback_block(keys, N, kA, kB, iA, iB, keys_sorted);
+}
+
 // ---- single-wave sort: every phase in one cooperative launch ---------------------------------------------------
 constexpr int kSmallDB = kSortDigitBits;   // 11-bit digits, at most three passes
 constexpr int kLargeDB = 9;                // 9-bit digits, at most four passes over 36 prefix bits
@@ -661,6 +742,9 @@ mex_sort_small_kernel(const __grid_constant__ SortParams P) {
     grid.sync();
     sort_phase_fixruns(P, pl, words, heads);
     ETICS_PROF();
+    grid.sync();
+    if (blockIdx.x == 0 && __ldcg(&P.hdr->fallback) != 0u)   // never taken by the paper's workloads
+        sort_fallback_block(P.keys, P.N, P.bufA, P.bufB, P.perm, P.itmp, P.keys_sorted);
 }
 
 // ---- bandwidth-bound sort: one kernel per phase; a pass beyond the plan's last one returns at once -----------------
@@ -708,79 +792,6 @@ mex_sort_fixruns_kernel(const __grid_constant__ SortParams P) {
     sort_phase_fixruns(P, pl, (pl.passes & 1) ? P.bufB : P.bufA, reinterpret_cast<const unsigned*>((pl.passes & 1) ? P.bufA : P.bufB));
 }
 
-// =========================================================================================================
-// Fallback: stable LSD sort of (full key, index), eight 8-bit passes, ONE block (histogram by all threads, stable
-// scatter by warp 0, 32 keys per step).  Runs only when the fix-up raised the flag.
-// =========================================================================================================
-__global__ void __launch_bounds__(1024)
-mex_sort_fallback_kernel(const SortHeader* __restrict__ hdr, const unsigned long long* __restrict__ keys, long long N,
-                         unsigned long long* kA, unsigned long long* kB, unsigned* iA, unsigned* iB,
-                         unsigned long long* keys_sorted) {
-    if (__ldcg(&hdr->fallback) == 0u) return;
-    __shared__ unsigned hist[256];
-    __shared__ unsigned base[256];
-    __shared__ int single;
-    const int tid = threadIdx.x, lane = tid & 31;
-    int cur = -1;   // -1: the source is (keys, identity); 0: set A; 1: set B
-    for (int pass = 0; pass < 8; ++pass) {
-        const int shift = 8 * pass;
-        const unsigned long long* ksrc = (cur < 0) ? keys : (cur == 0 ? kA : kB);
-        const unsigned* isrc = (cur < 0) ? nullptr : (cur == 0 ? iA : iB);
-        unsigned long long* kdst = (cur == 0) ? kB : kA;
-        unsigned* idst = (cur == 0) ? iB : iA;
-        if (tid < 256) hist[tid] = 0;
-        if (tid == 0) single = 0;
-        __syncthreads();
-        for (long long k = tid; k < N; k += 1024) atomicAdd(&hist[(unsigned)(ksrc[k] >> shift) & 255u], 1u);
-        __syncthreads();
-        if (tid < 256 && hist[tid] == (unsigned)N) single = 1;
-        __syncthreads();
-        const bool skip = single != 0 && cur >= 0;   // every key has the same digit: a stable pass would change nothing
-        __syncthreads();                              // `single` is rewritten at the top of the next pass
-        if (skip) continue;
-        if (tid == 0) {
-            unsigned run = 0;
-            for (int d = 0; d < 256; ++d) { base[d] = run; run += hist[d]; }
-        }
-        __syncthreads();
-        if (tid < 32) {
-            for (long long k0 = 0; k0 < N; k0 += 32) {
-                const long long k = k0 + lane;
-                const bool ok = k < N;
-                const unsigned long long key = ok ? ksrc[k] : 0ull;
-                const unsigned d = ok ? ((unsigned)(key >> shift) & 255u) : 256u;
-                unsigned peers = 0xffffffffu;
-#pragma unroll
-                for (int b = 0; b < 9; ++b) {
-                    const bool bit = (d >> b) & 1u;
-                    const unsigned vote = __ballot_sync(0xffffffffu, bit);
-                    peers &= bit ? vote : ~vote;
-                }
-                if (ok) {
-                    const unsigned lower = peers & ((1u << lane) - 1u);
-                    const unsigned g = base[d] + __popc(lower);
-                    kdst[g] = key;
-                    idst[g] = isrc ? isrc[k] : (unsigned)k;
-                }
-                __syncwarp();
-                if (ok && (peers & ((1u << lane) - 1u)) == 0u) base[d] += __popc(peers);
-                __syncwarp();
-            }
-        }
-        __threadfence();
-        __syncthreads();
-        cur = (cur == 0) ? 1 : 0;
-    }
-    // the result belongs in set A (iA is the caller's permutation)
-    if (cur == 1) {
-        for (long long k = tid; k < N; k += 1024) { kA[k] = kB[k]; iA[k] = iB[k]; }
-        __threadfence();
-        __syncthreads();
-    }
-    if (keys_sorted)
-        for (long long k = tid; k < N; k += 1024) keys_sorted[k] = kA[k];
-}
-
 // ---------------------------------------------------------------------------------------------------------
 // Host side.
 // ---------------------------------------------------------------------------------------------------------
@@ -815,13 +826,13 @@ static cudaError_t sort_device(SortDevice* out) {
     return cudaSuccess;
 }
 
-// kernels one sort launches (for the launch count bench.py reports): the cooperative kernel + the fallback kernel, or
+// kernels one sort launches (for the launch count bench.py reports): the cooperative kernel, or
 // keys + (histogram, scan, scatter) per pass + the two fix-up kernels + the fallback kernel
 int mex_sort_kernel_launches(long long N) {
     SortDevice dv;
     if (sort_device(&dv) != cudaSuccess) return 0;
     const long long tiles = (N + kSortTile - 1) / kSortTile;
-    return tiles <= dv.small_blocks ? 2 : 1 + 3 * (kLargePrefixBits / kLargeDB) + 2 + 1;
+    return tiles <= dv.small_blocks ? 1 : 1 + 3 * (kLargePrefixBits / kLargeDB) + 2 + 1;
 }
 
 cudaError_t mex_sort_init_device() {
@@ -845,6 +856,7 @@ cudaError_t mex_sort_enqueue(const double* pos, const double* mass, long long N,
     P.seg_hist = reinterpret_cast<unsigned*>(ws + L.off_seghist);
     P.bin_tot = reinterpret_cast<unsigned*>(ws + L.off_bintot);
     P.perm = perm_out; P.keys_sorted = keys_sorted_out;
+    P.itmp = reinterpret_cast<unsigned*>(ws + L.off_itmp);
     P.tiles = (N + kSortTile - 1) / kSortTile;
     e = cudaMemsetAsync(ws + L.off_hdr, 0, sizeof(SortHeader), st);
     if (e != cudaSuccess) return e;
@@ -861,6 +873,8 @@ cudaError_t mex_sort_enqueue(const double* pos, const double* mass, long long N,
         e = cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(mex_sort_small_kernel), dim3((unsigned)grid),
                                         dim3(kSortThreads), args, sizeof(SortSmem<kSmallDB>), st);
         if (e != cudaSuccess) return e;
+        if (ev_keygen) cudaEventRecord(ev_keygen, st);
+        return cudaSuccess;   // the fallback sort is the kernel's last phase
     } else {
         // Bandwidth-bound: one kernel per phase, a block per segment of consecutive tiles (two waves of segments), four
         // passes of 9-bit digits over 36 prefix bits — with 2048 digit values a tile of 4096 words would scatter runs of
@@ -885,8 +899,7 @@ cudaError_t mex_sort_enqueue(const double* pos, const double* mass, long long N,
         if (e != cudaSuccess) return e;
     }
     if (ev_keygen) cudaEventRecord(ev_keygen, st);
-    unsigned* itmp = reinterpret_cast<unsigned*>(ws + L.off_itmp);
-    mex_sort_fallback_kernel<<<1, 1024, 0, st>>>(P.hdr, P.keys, N, P.bufA, P.bufB, perm_out, itmp, keys_sorted_out);
+    mex_sort_fallback_kernel<<<1, 1024, 0, st>>>(P.hdr, P.keys, N, P.bufA, P.bufB, perm_out, P.itmp, keys_sorted_out);
     return cudaGetLastError();
 }
 
