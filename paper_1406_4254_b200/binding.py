@@ -23,7 +23,7 @@ ETICS_WHAT_BOTH, ETICS_WHAT_POTENTIAL, ETICS_WHAT_FORCE = 0, 1, 2
 # every symbol include/etics.h declares (tests check that the library exports all of them)
 EXPORTS = [
     "etics_status_string", "etics_init", "etics_workspace_bytes", "etics_scf_coeffs", "etics_scf_force",
-    "etics_mex_force", "etics_scf_force_ex", "etics_mex_force_ex", "etics_mex_sort", "etics_host_scratch_bytes", "etics_scf_full_host",
+    "etics_mex_force", "etics_scf_combine", "etics_scf_force_ex", "etics_mex_force_ex", "etics_mex_sort", "etics_host_scratch_bytes", "etics_scf_full_host",
     "etics_mex_full_host", "etics_mex_force_timed", "etics_probe_dfma", "etics_probe_copy",
     "etics_kernel_launches", "etics_step_host_scratch_bytes", "etics_step_host", "etics_stepper_workspace_bytes", "etics_stepper_create", "etics_stepper_step", "etics_stepper_set_coefficient_interval", "etics_stepper_destroy",
 ]
@@ -60,6 +60,8 @@ def lib() -> C.CDLL:
     L.etics_scf_force.argtypes = [_vp, _ll, _i, _i, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
     L.etics_mex_force.restype = _i
     L.etics_mex_force.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _vp, _sz, _vp]
+    L.etics_scf_combine.restype = _i
+    L.etics_scf_combine.argtypes = [_vp, _i, _ll, _vp, _vp]
     L.etics_scf_force_ex.restype = _i
     L.etics_scf_force_ex.argtypes = [_vp, _ll, _i, _i, _vp, _vp, _i, _vp, _vp, _vp, _sz, _vp]
     L.etics_mex_force_ex.restype = _i
@@ -182,6 +184,15 @@ def etics_mex_force(pos, mass, lmax: int, acc=None, pot=None, workspace=None, st
                               workspace.data_ptr(), wsb, _stream(stream))
     _check(s, "etics_mex_force")
     return acc, pot
+
+
+def etics_scf_combine(parts, out=None, stream=None):
+    """parts (R, len) CUDA fp64, the ranks' tables in rank order -> out (len,) = their sum in that order."""
+    R, n = parts.shape
+    if out is None:
+        out = torch.empty(n, dtype=torch.float64, device=parts.device)
+    _check(lib().etics_scf_combine(_dev(parts, "parts"), R, n, _dev(out, "out"), _stream(stream)), "etics_scf_combine")
+    return out
 
 
 def _opt(t, name):

@@ -97,6 +97,12 @@ etics_status etics_mex_force(const double* pos, const double* mass, long long N,
     return etics_mex_force_ex(pos, mass, N, lmax, ETICS_WHAT_BOTH, acc, pot, workspace, workspace_bytes, stream);
 }
 
+etics_status etics_scf_combine(const double* parts, int nparts, long long len, double* out, void* stream) {
+    if (!parts || !out || nparts < 1 || len < 1) return ETICS_ERR_ARG;
+    if (misaligned(parts) || misaligned(out)) return ETICS_ERR_ALIGN;
+    return from_cuda(scf_combine_launch(parts, nparts, len, out, static_cast<cudaStream_t>(stream)));
+}
+
 etics_status etics_mex_sort(const double* pos, long long N, unsigned long long* keys_sorted, unsigned int* perm,
                             void* workspace, size_t workspace_bytes, void* stream) {
     etics_status s = check_sizes(N, 0, 0);

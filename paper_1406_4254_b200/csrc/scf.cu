@@ -551,6 +551,22 @@ scf_finalize_kernel(const double* __restrict__ partial, int blocks, int nmax, in
     else B[tt] = norm * s;
 }
 
+// Sharded SCF (partial coefficients of every rank, then MPI_Allreduce): the tables of
+// all ranks, gathered in rank order, are added in THAT order — the same bits on every rank and in every run.
+__global__ void __launch_bounds__(256)
+scf_combine_kernel(const double* __restrict__ parts, int nparts, long long len, double* __restrict__ out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= len) return;
+    double s = parts[i];
+    for (int r = 1; r < nparts; ++r) s += parts[(size_t)r * len + i];
+    out[i] = s;
+}
+
+cudaError_t scf_combine_launch(const double* parts, int nparts, long long len, double* out, cudaStream_t st) {
+    scf_combine_kernel<<<(unsigned)((len + 255) / 256), 256, 0, st>>>(parts, nparts, len, out);
+    return cudaGetLastError();
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // Host side: plan, workspace, launches.
 // ---------------------------------------------------------------------------------------------------------

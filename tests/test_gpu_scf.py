@@ -205,3 +205,31 @@ def test_force_only_and_potential_only(E, nmax, lmax):
     assert rel_err_scalar(pot_p.cpu().numpy(), pot.cpu().numpy(), floor=0.0) <= 1e-14   # same sums, possibly another schedule
     assert E.lib().etics_scf_force_ex(dpos.data_ptr(), pos.shape[1], nmax, lmax, A.data_ptr(), B.data_ptr(), 3,
                                       acc.data_ptr(), pot.data_ptr(), None, 0, 0) == E.ETICS_ERR_ARG
+
+
+def test_sharded_scf_on_one_gpu_matches_the_whole(E):
+    """etics_scf_combine + the shard arithmetic of paper_1406_4254_b200.sharded, with both 'ranks' on this GPU one after the
+    other (no process group): shard tables added in rank order = coefficients of the whole set; shard evaluations = slices."""
+    from paper_1406_4254_b200 import sharded
+    n, nmax, lmax, world = 50_001, 10, 6, 3
+    pos, mass = W.particles("hernquist", n, seed=9, axes=(1.0, 0.8, 0.6))
+    T = (nmax + 1) * E.num_lm(lmax)
+    tables = torch.empty((world, 2 * T), dtype=torch.float64, device="cuda")
+    shards = []
+    for r in range(world):
+        a, b = sharded.shard_range(n, r, world)
+        dp, dm = dev(pos[:, a:b]), dev(mass[a:b])
+        E.etics_scf_coeffs(dp, dm, nmax, lmax, tables[r, :T], tables[r, T:])
+        shards.append((a, b, dp))
+    table = sharded.gather_and_combine(tables[0], lambda t: tables, E.etics_scf_combine)
+    A0, B0 = oracle.scf_coeffs(pos, mass, nmax, lmax)
+    assert rel_err_scalar(table[:T].cpu().numpy(), A0) <= TOL and rel_err_scalar(table[T:].cpu().numpy(), B0) <= TOL
+    expect = tables[0].clone()
+    for r in range(1, world):
+        expect += tables[r]
+    assert torch.equal(table, expect)                     # rank order, one addition per rank
+    acc0, pot0 = oracle.scf_force(pos, nmax, lmax, A0, B0)
+    for a, b, dp in shards:
+        acc, pot = E.etics_scf_force(dp, nmax, lmax, table[:T].contiguous(), table[T:].contiguous())
+        assert rel_err_vector(acc.cpu().numpy(), acc0[:, a:b]) <= TOL
+        assert rel_err_scalar(pot.cpu().numpy(), pot0[a:b], floor=0.0) <= TOL

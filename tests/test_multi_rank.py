@@ -68,3 +68,66 @@ def test_reference_arm_only_rank0_prints():
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["gpu_launches"] == 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
     assert d["value"] > 0 and d["unit"] == "particles/s"
+
+
+SHARD_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, os.environ["ETICS_ROOT"])
+import numpy as np
+import torch, torch.distributed as dist
+import oracle
+from paper_1406_4254_b200 import sharded, workloads as W
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+n, nmax, lmax = 2001, 6, 4
+pos, mass = W.particles("hernquist", n, seed=4, axes=(1.0, 0.8, 0.6))
+a, b = sharded.shard_range(n, rank, world)
+# the exchange logic of sharded.scf_force_sharded, with the oracle standing in for the kernels (no GPU here):
+A, B = oracle.scf_coeffs(np.ascontiguousarray(pos[:, a:b]), mass[a:b], nmax, lmax)
+local = torch.from_numpy(np.concatenate([A, B]))
+def all_gather(t):
+    stack = [torch.empty_like(t) for _ in range(world)]
+    dist.all_gather(stack, t)
+    return torch.stack(stack)
+def combine(stack):
+    s = stack[0].clone()
+    for r in range(1, stack.shape[0]):
+        s += stack[r]
+    return s
+table = sharded.gather_and_combine(local, all_gather, combine).numpy()
+T = len(A)
+acc, pot = oracle.scf_force(np.ascontiguousarray(pos[:, a:b]), nmax, lmax, table[:T], table[T:])
+A0, B0 = oracle.scf_coeffs(pos, mass, nmax, lmax)
+acc0, pot0 = oracle.scf_force(pos, nmax, lmax, A0, B0)
+print("RESULT " + json.dumps({"rank": rank, "first": a, "last": b,
+      "errA": float(np.max(np.abs(table[:T] - A0)) / np.max(np.abs(A0))),
+      "errpot": float(np.max(np.abs(pot - pot0[a:b]) / np.abs(pot0[a:b]))),
+      "digest": float(np.sum(table * np.arange(1, 2 * T + 1)))}), flush=True)
+dist.destroy_process_group()
+"""
+
+
+def test_shard_ranges_cover_every_particle_once():
+    from paper_1406_4254_b200 import sharded
+    for n in (0, 1, 7, 1000, 1001, 12345):
+        for world in (1, 2, 3, 8):
+            r = [sharded.shard_range(n, k, world) for k in range(world)]
+            assert r[0][0] == 0 and r[-1][1] == n
+            assert all(r[k][1] == r[k + 1][0] for k in range(world - 1))
+            sizes = [b - a for a, b in r]
+            assert max(sizes) - min(sizes) <= 1
+
+
+def test_sharded_scf_exchange_two_ranks(tmp_path):
+    """SURVEY 8(f)3 / PAPER.md:195, :221: coefficients of the shards, gathered and added in rank order, are the coefficients
+    of the whole set (to summation rounding), identical on both ranks; every rank's shard then gets the whole set's field."""
+    w = tmp_path / "shard_worker.py"
+    w.write_text(SHARD_WORKER)
+    r = _torchrun([str(w)])
+    assert r.returncode == 0, r.stderr[-2000:]
+    res = sorted((json.loads(m) for m in re.findall(r"RESULT (\{[^{}]*\})", r.stdout)), key=lambda x: x["rank"])
+    assert [x["rank"] for x in res] == [0, 1]
+    assert res[0]["first"] == 0 and res[0]["last"] == res[1]["first"] and res[1]["last"] == 2001
+    for x in res:
+        assert x["errA"] < 1e-13 and x["errpot"] < 1e-12
+    assert res[0]["digest"] == res[1]["digest"]          # bit-identical tables on both ranks
