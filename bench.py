@@ -445,6 +445,10 @@ def run_ours(args):
             "both": phases["scf_force_ms"],
             "potential_only": float(np.mean(timed(lambda: E.etics_scf_force_ex(pos, nmax, lmax, A, B, E.ETICS_WHAT_POTENTIAL, None, pot), k_iters, 2))),
             "force_only": float(np.mean(timed(lambda: E.etics_scf_force_ex(pos, nmax, lmax, A, B, E.ETICS_WHAT_FORCE, acc, None), k_iters, 2)))}
+        ws_f32 = torch.empty(E.etics_workspace_bytes(E.ETICS_WS_SCF_FORCE_F32, N, nmax, lmax), dtype=torch.uint8, device="cuda")
+        variants["scf_force_ms"]["both_fp32_arithmetic"] = float(np.mean(timed(
+            lambda: E.etics_scf_force_f32(pos, nmax, lmax, A, B, E.ETICS_WHAT_BOTH, acc, pot, ws_f32), k_iters, 2)))
+        scf_force()   # leave the fp64 results in acc, pot
     if mex_lmax is not None:
         variants["mex_force_ms"] = {
             "both": phases["mex_force_ms"],

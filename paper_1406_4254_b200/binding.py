@@ -17,13 +17,13 @@ LIB_PATH = os.path.join(HERE, "libetics.so")
 ETICS_OK = 0
 ETICS_ERR_ARG, ETICS_ERR_LIMIT, ETICS_ERR_ALIGN, ETICS_ERR_WORKSPACE, ETICS_ERR_CUDA = -1, -2, -3, -4, -5
 ETICS_MAX_LMAX, ETICS_MAX_NMAX = 10, 32
-ETICS_WS_SCF_COEFFS, ETICS_WS_SCF_FORCE, ETICS_WS_MEX_FORCE = 0, 1, 2
+ETICS_WS_SCF_COEFFS, ETICS_WS_SCF_FORCE, ETICS_WS_MEX_FORCE, ETICS_WS_SCF_FORCE_F32 = 0, 1, 2, 3
 ETICS_WHAT_BOTH, ETICS_WHAT_POTENTIAL, ETICS_WHAT_FORCE = 0, 1, 2
 
 # every symbol include/etics.h declares (tests check that the library exports all of them)
 EXPORTS = [
     "etics_status_string", "etics_init", "etics_workspace_bytes", "etics_scf_coeffs", "etics_scf_force",
-    "etics_mex_force", "etics_scf_combine", "etics_scf_force_ex", "etics_mex_force_ex", "etics_mex_sort", "etics_host_scratch_bytes", "etics_scf_full_host",
+    "etics_mex_force", "etics_scf_combine", "etics_scf_force_f32", "etics_scf_force_ex", "etics_mex_force_ex", "etics_mex_sort", "etics_host_scratch_bytes", "etics_scf_full_host",
     "etics_mex_full_host", "etics_mex_force_timed", "etics_probe_dfma", "etics_probe_copy",
     "etics_kernel_launches", "etics_step_host_scratch_bytes", "etics_step_host", "etics_stepper_workspace_bytes", "etics_stepper_create", "etics_stepper_step", "etics_stepper_set_coefficient_interval", "etics_stepper_destroy",
 ]
@@ -60,6 +60,8 @@ def lib() -> C.CDLL:
     L.etics_scf_force.argtypes = [_vp, _ll, _i, _i, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
     L.etics_mex_force.restype = _i
     L.etics_mex_force.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _vp, _sz, _vp]
+    L.etics_scf_force_f32.restype = _i
+    L.etics_scf_force_f32.argtypes = [_vp, _ll, _i, _i, _vp, _vp, _i, _vp, _vp, _vp, _sz, _vp]
     L.etics_scf_combine.restype = _i
     L.etics_scf_combine.argtypes = [_vp, _i, _ll, _vp, _vp]
     L.etics_scf_force_ex.restype = _i
@@ -209,6 +211,20 @@ def etics_scf_force_ex(pos, nmax: int, lmax: int, A, B, what: int, acc=None, pot
     s = lib().etics_scf_force_ex(_dev(pos, "pos"), N, nmax, lmax, _dev(A, "A"), _dev(B, "B"), what, _opt(acc, "acc"),
                                  _opt(pot, "pot"), None, 0, _stream(stream))
     _check(s, "etics_scf_force_ex")
+    return (None if what == ETICS_WHAT_POTENTIAL else acc), (None if what == ETICS_WHAT_FORCE else pot)
+
+
+def etics_scf_force_f32(pos, nmax: int, lmax: int, A, B, what: int = ETICS_WHAT_BOTH, acc=None, pot=None, workspace=None, stream=None):
+    """Single-precision evaluation (fp64 arrays in and out); see include/etics.h."""
+    N = pos.shape[1]
+    if acc is None and what != ETICS_WHAT_POTENTIAL:
+        acc = torch.empty((3, N), dtype=torch.float64, device=pos.device)
+    if pot is None and what != ETICS_WHAT_FORCE:
+        pot = torch.empty(N, dtype=torch.float64, device=pos.device)
+    workspace, wsb = _workspace(ETICS_WS_SCF_FORCE_F32, N, nmax, lmax, pos.device, workspace)
+    s = lib().etics_scf_force_f32(_dev(pos, "pos"), N, nmax, lmax, _dev(A, "A"), _dev(B, "B"), what, _opt(acc, "acc"),
+                                  _opt(pot, "pot"), workspace.data_ptr(), wsb, _stream(stream))
+    _check(s, "etics_scf_force_f32")
     return (None if what == ETICS_WHAT_POTENTIAL else acc), (None if what == ETICS_WHAT_FORCE else pot)
 
 

@@ -46,6 +46,7 @@ size_t etics_workspace_bytes(int which, long long N, int nmax, int lmax) {
         case ETICS_WS_SCF_COEFFS: b = scf_coeffs_workspace(N, nmax, lmax); break;
         case ETICS_WS_SCF_FORCE: b = 0; break;
         case ETICS_WS_MEX_FORCE: b = mex_workspace(N, lmax); break;
+        case ETICS_WS_SCF_FORCE_F32: b = scf_force_f32_workspace(nmax, lmax); break;
         default: return 0;
     }
     return b < 256 ? 256 : round_up(b, 256);
@@ -95,6 +96,19 @@ etics_status etics_mex_force_ex(const double* pos, const double* mass, long long
 etics_status etics_mex_force(const double* pos, const double* mass, long long N, int lmax,
                              double* acc, double* pot, void* workspace, size_t workspace_bytes, void* stream) {
     return etics_mex_force_ex(pos, mass, N, lmax, ETICS_WHAT_BOTH, acc, pot, workspace, workspace_bytes, stream);
+}
+
+etics_status etics_scf_force_f32(const double* pos, long long N, int nmax, int lmax, const double* A, const double* B,
+                                 int what, double* acc, double* pot, void* workspace, size_t workspace_bytes, void* stream) {
+    etics_status s = check_sizes(N, nmax, lmax);
+    if (s != ETICS_OK) return s;
+    if (what != ETICS_WHAT_BOTH && what != ETICS_WHAT_POTENTIAL && what != ETICS_WHAT_FORCE) return ETICS_ERR_ARG;
+    if (what == ETICS_WHAT_POTENTIAL) acc = nullptr;
+    if (what == ETICS_WHAT_FORCE) pot = nullptr;
+    if (!pos || !A || !B || !workspace || (!acc && what != ETICS_WHAT_POTENTIAL) || (!pot && what != ETICS_WHAT_FORCE)) return ETICS_ERR_ARG;
+    if (misaligned(pos) || misaligned(A) || misaligned(B) || misaligned(acc) || misaligned(pot) || misaligned(workspace)) return ETICS_ERR_ALIGN;
+    if (workspace_bytes < etics_workspace_bytes(ETICS_WS_SCF_FORCE_F32, N, nmax, lmax)) return ETICS_ERR_WORKSPACE;
+    return from_cuda(scf_force_f32_launch(pos, N, nmax, lmax, A, B, acc, pot, workspace, static_cast<cudaStream_t>(stream)));
 }
 
 etics_status etics_scf_combine(const double* parts, int nparts, long long len, double* out, void* stream) {

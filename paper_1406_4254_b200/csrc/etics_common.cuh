@@ -200,6 +200,9 @@ cudaError_t scf_finalize_launch(long long N, int nmax, int lmax, double* A, doub
 cudaError_t scf_force_launch(const double* pos, long long N, int nmax, int lmax, const double* A, const double* B, int what,
                              double* acc, double* pot, cudaStream_t st);
 
+size_t scf_force_f32_workspace(int nmax, int lmax);
+cudaError_t scf_force_f32_launch(const double* pos, long long N, int nmax, int lmax, const double* A, const double* B,
+                                 double* acc, double* pot, void* ws, cudaStream_t st);
 cudaError_t scf_combine_launch(const double* parts, int nparts, long long len, double* out, cudaStream_t st);
 
 cudaError_t mex_init_constants();

@@ -89,7 +89,7 @@ def test_workspace_sizes(libetics):
         for n in (1, 10_000, 1_000_000, 100_000_000):
             b = f(which, n, 10, 6)
             assert b >= 256 and b % 256 == 0
-    assert f(3, 1000, 10, 6) == 0
+    assert f(4, 1000, 10, 6) == 0
     assert f(0, 0, 10, 6) == 0
     assert f(2, 1000, 10, 11) == 0
     # MEX workspace grows with N (sort double-buffers + sorted records), SCF coefficient workspace is bounded

@@ -233,3 +233,44 @@ def test_sharded_scf_on_one_gpu_matches_the_whole(E):
         acc, pot = E.etics_scf_force(dp, nmax, lmax, table[:T].contiguous(), table[T:].contiguous())
         assert rel_err_vector(acc.cpu().numpy(), acc0[:, a:b]) <= TOL
         assert rel_err_scalar(pot.cpu().numpy(), pot0[a:b], floor=0.0) <= TOL
+
+
+F32_TOL_POT, F32_TOL_ACC = 1e-4, 1e-3   # fp32 eps 6e-8 x the ~1e3 cancellation of the mixed-sign sums over (n, l, m); see DESIGN.md
+
+
+@pytest.mark.parametrize("nmax,lmax", [(10, 6), (20, 10), (6, 2), (0, 0)])
+def test_f32_mode_against_the_fp64_oracle(E, nmax, lmax):
+    """single-precision evaluation; coefficients from the fp64 path."""
+    pos, mass = W.particles("hernquist", 20_011, seed=17, axes=(1.0, 0.8, 0.6))
+    dpos, dmass = dev(pos), dev(mass)
+    A, B = E.etics_scf_coeffs(dpos, dmass, nmax, lmax)
+    acc, pot = E.etics_scf_force_f32(dpos, nmax, lmax, A, B)
+    _, pot_only = E.etics_scf_force_f32(dpos, nmax, lmax, A, B, E.ETICS_WHAT_POTENTIAL)
+    acc_only, _ = E.etics_scf_force_f32(dpos, nmax, lmax, A, B, E.ETICS_WHAT_FORCE)
+    torch.cuda.synchronize()
+    A0, B0 = oracle.scf_coeffs(pos, mass, nmax, lmax)
+    acc0, pot0 = oracle.scf_force(pos, nmax, lmax, A0, B0)
+    ep, ea = rel_err_scalar(pot.cpu().numpy(), pot0, floor=0.0), rel_err_vector(acc.cpu().numpy(), acc0)
+    assert ep <= F32_TOL_POT and ea <= F32_TOL_ACC, (ep, ea)
+    assert ep > 1e-9          # it really is single precision
+    assert torch.equal(pot_only, pot) and torch.equal(acc_only, acc)
+
+
+def test_f32_mode_is_accurate_near_the_z_axis(E):
+    """the paper's fp32 runs fail near the z axis (eq. 24); the l-recurrence at fixed m does not."""
+    nmax, lmax = 10, 6
+    pos, mass = W.config_particles(1)
+    A, B = E.etics_scf_coeffs(dev(pos), dev(mass), nmax, lmax)
+    # field points: on the axis, and 1e-7 ... 1e-2 rad off it, both poles, several radii
+    th = np.array([0.0, 1e-7, 1e-5, 1e-4, 1e-3, 1e-2])
+    th = np.concatenate([th, np.pi - th])
+    r = np.array([0.05, 0.7, 3.0, 40.0])
+    T, R = np.meshgrid(th, r, indexing="ij")
+    ph = 0.3 + 1.7 * np.arange(T.size)
+    pts = np.stack([(R * np.sin(T)).ravel() * np.cos(ph), (R * np.sin(T)).ravel() * np.sin(ph), (R * np.cos(T)).ravel()])
+    acc, pot = E.etics_scf_force_f32(dev(pts), nmax, lmax, A, B)
+    torch.cuda.synchronize()
+    A0, B0 = oracle.scf_coeffs(pos, mass, nmax, lmax)
+    acc0, pot0 = oracle.scf_force(pts, nmax, lmax, A0, B0)
+    assert rel_err_scalar(pot.cpu().numpy(), pot0, floor=0.0) <= F32_TOL_POT
+    assert rel_err_vector(acc.cpu().numpy(), acc0) <= F32_TOL_ACC
