@@ -1,34 +1,30 @@
 // mex.cu — MEX half of the hot path (SURVEY.md §8(a) M1–M7) for sm_100a.
 //
-//   mex_keygen_kernel      M1: key = bits(r^2) (rounding pinned: t=x*x; t=fma(y,y,t); t=fma(z,z,t)), idx = k, and the
-//                          256-bin histograms of all eight key bytes in the same pass.
-//   mex_radix_pass_kernel  M2: one stable LSD pass over 8 key bits, "onesweep" style: each tile ranks its keys with
-//                          warp match/popc, reorders them in shared memory, obtains its global bucket offsets by a
-//                          decoupled lookback over the preceding tiles' per-digit counts (integers: exact, so the
-//                          result does not depend on timing) and writes keys + payload once.  Hand-written, no CUB.
-//   mex_gather_kernel      M3: sorted order -> per-particle geometry records (r, 1/r, cos/sin theta, cos/sin phi, m)
-//                          in a chunk-transposed SoA layout that the scan kernels read fully coalesced.
-//   mex_aggregate_kernel   M4+M5a: every thread owns K consecutive sorted particles and sums their moments
-//                          w_lm m r^l P_lm {cos,sin} m phi and w_lm m r^-(l+1) P_lm {cos,sin} m phi; block-level
-//                          exclusive scan (inside-out for q, outside-in for p) in shared memory; per-chunk prefixes
-//                          and per-tile totals to the workspace.
+//   (mex_sort.cu)          M1-M2: keys = bits(r^2) (rounding pinned: t=x*x; t=fma(y,y,t); t=fma(z,z,t)), packed (x,y,z,m)
+//                          records, stable radial sort -> permutation.
+//   mex_gather_totals_kernel  M3+M4: sorted order -> per-particle geometry records (r, 1/r, cos/sin theta, cos/sin phi, m)
+//                          in a chunk-transposed SoA layout that the scan kernels read fully coalesced; every lane
+//                          owns K consecutive sorted particles, sums their moments m r^l P_lm {cos,sin} m phi and
+//                          m r^-(l+1) P_lm {cos,sin} m phi, and the warp adds the 32 chunk sums: tile totals.
 //   mex_tilescan_kernel    M5b: exclusive scan of the tile totals (forward for q, backward for p), fixed order.
-//   mex_evaluate_kernel    M5c+M6+M7: each thread re-walks its K particles forwards carrying q and backwards
-//                          carrying p (never "total minus prefix": that cancels catastrophically), accumulates
-//                          potential and spherical force components, transforms to Cartesian and scatters to the
-//                          particle's original index.
+//   mex_evaluate_kernel    M5a+M5c+M6+M7: each lane recomputes its chunk sums, the warp scans them in shared memory
+//                          (inside-out for q, outside-in for p), then each lane re-walks its K particles forwards
+//                          carrying q and backwards carrying p (never "total minus prefix": that cancels
+//                          catastrophically), accumulates potential and spherical force components, transforms
+//                          to Cartesian and scatters one 32-byte record to the particle's original index.
+//   mex_unpack_kernel      records -> acc (3,N), pot (N).
 //
 // The fp64 scans use a fixed summation order (thread chunk -> tile -> grid), so results are bitwise reproducible.
 // The (l,m) set is split into groups of whole m-columns (the Legendre l-recurrence runs along a column), so a
-// thread never holds more than ~17 (l,m) pairs of running sums in registers at a time.
+// thread never holds more than 28 running sums per direction in registers at a time.
 //
 // What the paper did instead (prior art, §3.2): Thrust merge sort of particle structs, a cache
 // kernel, then per l: a summand kernel writing q_lm, p_lm of every particle to global memory, one Thrust
 // exclusive_scan per (m, re/im, direction), a partial-force kernel; finally a coordinate-transform kernel.
 #include "mex_common.cuh"
 
-// This file is compiled four times (paper_1406_4254_b200/build.py) with ETICS_MEX_PART = 0..3: part 0 holds the sort,
-// the host entry points and the scan kernels for lmax <= 6; parts 1-3 only instantiate the scan kernels for lmax 7-8, 9
+// This file is compiled four times (paper_1406_4254_b200/build.py) with ETICS_MEX_PART = 0..3: part 0 holds the workspace
+// layout, the host entry points and the scan kernels for lmax <= 6; parts 1-3 only instantiate the scan kernels for lmax 7-8, 9
 // and 10 — the template instances dominate the compile time and the parts build in parallel.
 #ifndef ETICS_MEX_PART
 #define ETICS_MEX_PART 0

@@ -12,7 +12,7 @@ constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kSortDigitBits = 11;                 // widest digit of a pass
 constexpr int kSortBins = 1 << kSortDigitBits;     // 2048
 constexpr int kSortMaxPasses = 3;
-constexpr int kSortPrefixBits = kSortDigitBits * kSortMaxPasses;   // 33 key bits are radix-sorted, the rest is fixed up
+constexpr int kSortPrefixBits = kSortDigitBits * kSortMaxPasses;   // single-wave sort: 33 key bits are radix-sorted, the rest is fixed up
 constexpr int kSortMinTile = kSortThreads * 16;    // words per sort tile
 constexpr int kSortMaxSegs = 1024;                 // blocks of the persistent sort kernel (segment histogram rows)
 
