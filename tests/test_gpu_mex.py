@@ -118,6 +118,30 @@ def test_sort_prefix_collisions_long_runs_fallback(E):
     check_sort(E, pos)
 
 
+def _pad_to_bandwidth_bound_path(pos, n_total, seed):
+    """The same clusters inside a set large enough (> ~1.2e6) for the one-kernel-per-phase sort (36 prefix bits, 9-bit digits)."""
+    filler, _ = W.particles("hernquist", n_total - pos.shape[1], seed=seed)
+    rng = np.random.default_rng(seed)
+    allp = np.concatenate([pos, filler], axis=1)
+    return np.ascontiguousarray(allp[:, rng.permutation(allp.shape[1])])
+
+
+def test_sort_large_path_collisions_and_fallback(E):
+    """The sort for N above one tile per resident block: short runs for the two-phase fix-up, exact duplicates, all-equal
+    keys, and runs too long for the fix-up (fallback sort)."""
+    rng = np.random.default_rng(15)
+    pos = _pad_to_bandwidth_bound_path(_wide_range_with_clusters(rng.integers(2, 33, 3000), 2e-14, seed=16), 1_400_000, 17)
+    keys0, _ = oracle.mex_sort(pos)
+    assert np.sum((keys0[1:] >> np.uint64(27)) == (keys0[:-1] >> np.uint64(27))) > 20_000
+    check_sort(E, pos)
+    pos[:, 1000:1200] = pos[:, 999:1000]                     # 201 exact copies: a run the fix-up cannot order -> fallback
+    check_sort(E, pos)
+    pos = _pad_to_bandwidth_bound_path(_wide_range_with_clusters([4000, 64], 1e-15, seed=18), 1_300_001, 19)
+    check_sort(E, pos)
+    pos = np.zeros((3, 1_250_000)); pos[1] = 0.75             # every key equal: zero passes, pure stability
+    check_sort(E, pos)
+
+
 def test_sort_narrow_range_is_exact_without_fixup(E):
     """A thin shell: the whole key range fits the sorted prefix (shift = 0), whatever N."""
     rng = np.random.default_rng(11)

@@ -81,6 +81,16 @@ def test_graph_replay_is_bit_identical_and_steps_compose(E, method, nmax, lmax):
         assert np.array_equal(p, g) and np.array_equal(p, s)
 
 
+def test_graph_replay_large_sort_path(E):
+    """N above one sort tile per resident block: the step's graph holds the one-kernel-per-phase sort (20 MEX launches)."""
+    pos, vel, mass = initial_conditions(1_300_003, 16)
+    plain = run_gpu(E, 1, pos, vel, mass, 0.002, 3, 0, 2, False)
+    graph = run_gpu(E, 1, pos, vel, mass, 0.002, 3, 0, 2, True)
+    for p, g in zip(plain, graph):
+        assert np.array_equal(p, g)
+    assert np.all(np.isfinite(graph[0])) and np.all(np.isfinite(graph[2]))
+
+
 def test_stepper_argument_errors(E):
     import ctypes as C
     pos, vel, mass = initial_conditions(100, 1)
