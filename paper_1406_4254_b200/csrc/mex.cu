@@ -364,13 +364,25 @@ __device__ __forceinline__ void mex_chunk_sums(const double* rec_tile, int c, do
     constexpr int NS = mex_group_slots(LMAX, G);
 #pragma unroll
     for (int s = 0; s < NS; ++s) { q[s] = 0.0; pq[s] = 0.0; }
-    Rec p = CG ? load_rec_cg(rec_tile, 0, c) : load_rec(rec_tile, 0, c);
-#pragma unroll(LMAX <= 6 ? 1 : 2)
-    for (int k = 0; k < kMexK; ++k) {
-        const int kn = (k + 1 < kMexK) ? k + 1 : k;
-        const Rec nx = CG ? load_rec_cg(rec_tile, kn, c) : load_rec(rec_tile, kn, c);
-        mex_agg_particle<LMAX, G>(p, q, pq);
-        p = nx;
+    // the next record (lmax >= 7: the next two) is loaded while the current one is processed: a particle's moments are 270-450
+    // fp64 operations, about an L2 round trip with three warps per scheduler (two ahead at lmax 6 costs registers: spills)
+    auto ld = [&](int k) { return CG ? load_rec_cg(rec_tile, k < kMexK ? k : kMexK - 1, c) : load_rec(rec_tile, k < kMexK ? k : kMexK - 1, c); };
+    if constexpr (LMAX >= 7) {
+        Rec p = ld(0), n1 = ld(1);
+#pragma unroll 2
+        for (int k = 0; k < kMexK; ++k) {
+            const Rec n2 = ld(k + 2);
+            mex_agg_particle<LMAX, G>(p, q, pq);
+            p = n1; n1 = n2;
+        }
+    } else {
+        Rec p = ld(0);
+#pragma unroll 1
+        for (int k = 0; k < kMexK; ++k) {
+            const Rec n1 = ld(k + 1);
+            mex_agg_particle<LMAX, G>(p, q, pq);
+            p = n1;
+        }
     }
     mex_weight_sums<LMAX, G>(q, pq);
 }
@@ -520,6 +532,12 @@ __device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ re
     static_assert(NS <= kMexThreads, "one lane per row in the chunk scan");
     const int c = threadIdx.x;
     double s[NS];
+    // the tile's scanned totals of this lane's rows, asked for now and used after the chunk sums (volatile: not sunk to the use)
+    double tq = 0.0, tp = 0.0;
+    if (c < NS) {
+        asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(tq) : "l"(tot + (size_t)(RB + c) * tiles + tile));
+        asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(tp) : "l"(tot + (size_t)(RB + NS + c) * tiles + tile));
+    }
     // M5a: chunk sums (recomputed, never stored in HBM), then the exclusive scans along the 32 chunks of the tile in shared
     // memory, lane = row, serial in chunk order (q rows inside-out, p rows outside-in; the loads do not depend on the
     // running sum, so the chain is 32 DADDs).  The p prefixes wait in V while the forward walk runs.
@@ -534,7 +552,7 @@ __device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ re
             double x[kMexThreads];
 #pragma unroll
             for (int j = 0; j < kMexThreads; ++j) x[j] = v[j];
-            double run = tot[(size_t)(RB + c) * tiles + tile];   // the tile's exclusive prefix over the preceding tiles
+            double run = tq;   // the tile's exclusive prefix over the preceding tiles
 #pragma unroll
             for (int j = 0; j < kMexThreads; ++j) { v[j] = run; run += x[j]; }
         }
@@ -550,7 +568,7 @@ __device__ __forceinline__ void mex_evaluate_group(const double* __restrict__ re
             double x[kMexThreads];
 #pragma unroll
             for (int j = 0; j < kMexThreads; ++j) x[j] = v[j];
-            double run = tot[(size_t)(RB + NS + c) * tiles + tile];
+            double run = tp;
 #pragma unroll
             for (int j = kMexThreads - 1; j >= 0; --j) { v[j] = run; run += x[j]; }
         }
@@ -607,6 +625,11 @@ mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__
     const long long tile = blockIdx.x;
     const int c = threadIdx.x;
     const double* rec_tile = rec + (size_t)tile * kRecFields * kMexTile;
+    // the tile's records (7 fields x 256 doubles = 112 lines) are on their way before the first chunk sum asks for them
+    // (N = 1e6: 120.2 -> 116.2 us)
+#pragma unroll
+    for (int i = c; i < 7 * kMexTile / 16; i += kMexThreads)
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(rec_tile + 16 * i));
 #pragma unroll
     for (int i = 0; i < kMexK * 4; ++i) sOut[i * kMexThreads + c] = 0.0;   // lane-private column: no barrier needed
     constexpr int NG = mex_num_groups(LMAX);
@@ -618,24 +641,35 @@ mex_evaluate_kernel(const double* __restrict__ rec, const unsigned* __restrict__
     if constexpr (NG > 5) mex_evaluate_group<LMAX, 5, PO>(rec_tile, sOut, V, tot, tiles, tile);
     if constexpr (NG > 6) mex_evaluate_group<LMAX, 6, PO>(rec_tile, sOut, V, tot, tiles, tile);
     if constexpr (NG > 7) mex_evaluate_group<LMAX, 7, PO>(rec_tile, sOut, V, tot, tiles, tile);
-#pragma unroll 1
+    // M7: transform and scatter.  All indices and the four angle fields of the chunk's records are loaded first (the sums are
+    // dead, the registers are free): with one particle at a time every iteration waited out a full L2 round trip (ncu: 17 % of the
+    // kernel's stall samples sat on this loop's first arithmetic).
+    unsigned idx[kMexK];
+    double gct[kMexK], gst[kMexK], gcp[kMexK], gsp[kMexK];
+#pragma unroll
+    for (int k = 0; k < kMexK; ++k) {
+        idx[k] = idxT[(size_t)tile * kMexTile + k * kMexThreads + c];
+        if (!PO) {
+            const double* b = rec_tile + k * kMexThreads + c;
+            gct[k] = b[2 * kMexTile]; gst[k] = b[3 * kMexTile]; gcp[k] = b[4 * kMexTile]; gsp[k] = b[5 * kMexTile];
+        }
+    }
+#pragma unroll
     for (int k = 0; k < kMexK; ++k) {
         const long long p = tile * kMexTile + (long long)c * kMexK + k;
         if (p >= N) continue;
-        const unsigned i = idxT[(size_t)tile * kMexTile + k * kMexThreads + c];
         if (PO) {   // out4 is the caller's pot array: one 8-byte store at the original index
-            out4[i] = sOut[(k * 4 + 0) * kMexThreads + c];
+            out4[idx[k]] = sOut[(k * 4 + 0) * kMexThreads + c];
             continue;
         }
-        const Rec r = load_rec(rec_tile, k, c);
         Geom g;
-        g.r = r.r; g.rinv = r.rinv; g.ct = r.ct; g.st = r.st; g.cp = r.cp; g.sp = r.sp;
+        g.r = 0.0; g.rinv = 0.0; g.ct = gct[k]; g.st = gst[k]; g.cp = gcp[k]; g.sp = gsp[k];
         double ax, ay, az;
         to_cartesian(g, sOut[(k * 4 + 1) * kMexThreads + c], sOut[(k * 4 + 2) * kMexThreads + c],
                      sOut[(k * 4 + 3) * kMexThreads + c], ax, ay, az);
         // ONE full 32-byte sector per particle at its original index (four 8-byte stores into the SoA outputs cost
         // 22 us of the kernel's 120 at N = 10^6 and 5 of 22 ms at N = 10^8); mex_unpack_kernel streams it into acc, pot
-        st_global_v4(out4 + 4 * (size_t)i, sOut[(k * 4 + 0) * kMexThreads + c], ax, ay, az);
+        st_global_v4(out4 + 4 * (size_t)idx[k], sOut[(k * 4 + 0) * kMexThreads + c], ax, ay, az);
     }
 }
 
