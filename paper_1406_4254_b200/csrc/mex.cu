@@ -401,15 +401,12 @@ __device__ __forceinline__ void mex_totals_group(const double* rec_tile, double*
     __syncwarp();
     for (int row = c; row < ROWS; row += kMexThreads) {
         const double* v = V + row * kVStride;
-        double run = 0.0;
-        if (row < NS) {
+        // four interleaved partial sums (chunks j = 0, 4, 8, ...; 1, 5, ...; ...), then a fixed tree: a quarter of the
+        // dependent-add chain of a serial row sum, the same order in every run
+        double r0 = 0.0, r1 = 0.0, r2 = 0.0, r3 = 0.0;
 #pragma unroll
-            for (int j = 0; j < kMexThreads; ++j) run += v[j];
-        } else {
-#pragma unroll
-            for (int j = kMexThreads - 1; j >= 0; --j) run += v[j];
-        }
-        tot[(size_t)(RB + row) * tiles + tile] = run;
+        for (int j = 0; j < kMexThreads; j += 4) { r0 += v[j]; r1 += v[j + 1]; r2 += v[j + 2]; r3 += v[j + 3]; }
+        tot[(size_t)(RB + row) * tiles + tile] = (r0 + r1) + (r2 + r3);
     }
     __syncwarp();
 }
