@@ -16,7 +16,9 @@ LIB_PATH = os.path.join(HERE, "libetics.so")
 
 ETICS_OK = 0
 ETICS_ERR_ARG, ETICS_ERR_LIMIT, ETICS_ERR_ALIGN, ETICS_ERR_WORKSPACE, ETICS_ERR_CUDA = -1, -2, -3, -4, -5
+ETICS_ERR_STATIC_LIMIT = -6
 ETICS_MAX_LMAX, ETICS_MAX_NMAX = 10, 32
+ETICS_STATIC_MAX_TABLE = 1386
 ETICS_WS_SCF_COEFFS, ETICS_WS_SCF_FORCE, ETICS_WS_MEX_FORCE, ETICS_WS_SCF_FORCE_F32 = 0, 1, 2, 3
 ETICS_WHAT_BOTH, ETICS_WHAT_POTENTIAL, ETICS_WHAT_FORCE = 0, 1, 2
 
@@ -26,6 +28,7 @@ EXPORTS = [
     "etics_mex_force", "etics_scf_combine", "etics_scf_force_f32", "etics_scf_force_ex", "etics_mex_force_ex", "etics_mex_sort", "etics_host_scratch_bytes", "etics_scf_full_host",
     "etics_mex_full_host", "etics_mex_force_timed", "etics_probe_dfma", "etics_probe_copy",
     "etics_kernel_launches", "etics_step_host_scratch_bytes", "etics_step_host", "etics_stepper_workspace_bytes", "etics_stepper_create", "etics_stepper_step", "etics_stepper_set_coefficient_interval", "etics_stepper_destroy",
+    "etics_scf_coeffs_static_max_table", "etics_scf_coeffs_static",
 ]
 
 _lib = None
@@ -56,6 +59,10 @@ def lib() -> C.CDLL:
     L.etics_workspace_bytes.argtypes = [_i, _ll, _i, _i]
     L.etics_scf_coeffs.restype = _i
     L.etics_scf_coeffs.argtypes = [_vp, _vp, _ll, _i, _i, _vp, _vp, _vp, _sz, _vp]
+    L.etics_scf_coeffs_static_max_table.restype = _sz
+    L.etics_scf_coeffs_static_max_table.argtypes = []
+    L.etics_scf_coeffs_static.restype = _i
+    L.etics_scf_coeffs_static.argtypes = [_vp, _vp, _ll, _i, _i, _vp, _vp, _vp]
     L.etics_scf_force.restype = _i
     L.etics_scf_force.argtypes = [_vp, _ll, _i, _i, _vp, _vp, _vp, _vp, _vp, _sz, _vp]
     L.etics_mex_force.restype = _i
@@ -155,6 +162,23 @@ def etics_scf_coeffs(pos, mass, nmax: int, lmax: int, A=None, B=None, workspace=
     s = lib().etics_scf_coeffs(_dev(pos, "pos"), _dev(mass, "mass"), N, nmax, lmax, _dev(A, "A"), _dev(B, "B"),
                                workspace.data_ptr(), wsb, _stream(stream))
     _check(s, "etics_scf_coeffs")
+    return A, B
+
+
+def etics_scf_coeffs_static_max_table() -> int:
+    """Largest T = (nmax+1) * num_lm(lmax) etics_scf_coeffs_static accepts."""
+    return int(lib().etics_scf_coeffs_static_max_table())
+
+
+def etics_scf_coeffs_static(pos, mass, nmax: int, lmax: int, A, B, stream=None):
+    """etics_scf_coeffs with the block partials in the library's own __device__ array: no workspace, nothing allocated
+    (neither here: the caller passes A, B (T,) CUDA fp64).  T <= ETICS_STATIC_MAX_TABLE.  See include/etics.h."""
+    N = mass.shape[0]
+    T = (nmax + 1) * num_lm(lmax)
+    assert pos.shape == (3, N) and A.shape == (T,) and B.shape == (T,)
+    s = lib().etics_scf_coeffs_static(_dev(pos, "pos"), _dev(mass, "mass"), N, nmax, lmax, _dev(A, "A"), _dev(B, "B"),
+                                      _stream(stream))
+    _check(s, "etics_scf_coeffs_static")
     return A, B
 
 

@@ -19,7 +19,8 @@ LIB = os.path.join(HERE, "libetics.so")
 # (source, object stem, extra flags).  mex.cu is compiled in four parts (ETICS_MEX_PART: sort + lmax <= 6 | 7-8 | 9 | 10):
 # its template instances dominate the build and the parts compile in parallel.
 SOURCES = [("etics_api.cu", "etics_api", []), ("scf.cu", "scf", []), ("probe.cu", "probe", []), ("mex_sort.cu", "mex_sort", []),
-           ("stepper.cu", "stepper", []), ("scf_f32.cu", "scf_f32", [])] + \
+           ("stepper.cu", "stepper", []), ("scf_f32.cu", "scf_f32", []),
+           ("scf_static.cu", "scf_static", [])] + \
           [("mex.cu", f"mex_p{k}", [f"-DETICS_MEX_PART={k}"]) for k in range(4)]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

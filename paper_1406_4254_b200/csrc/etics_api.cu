@@ -28,6 +28,8 @@ const char* etics_status_string(etics_status s) {
         case ETICS_ERR_ALIGN: return "ETICS_ERR_ALIGN: pointer not 16-byte aligned";
         case ETICS_ERR_WORKSPACE: return "ETICS_ERR_WORKSPACE: workspace too small";
         case ETICS_ERR_CUDA: return "ETICS_ERR_CUDA: CUDA runtime or launch error";
+        case ETICS_ERR_STATIC_LIMIT:
+            return "ETICS_ERR_STATIC_LIMIT: (nmax+1)(lmax+1)(lmax+2)/2 beyond ETICS_STATIC_MAX_TABLE (1386) of etics_scf_coeffs_static";
         default: return "ETICS: unknown status";
     }
 }

@@ -49,7 +49,7 @@ def test_status_strings(libetics):
     libetics.etics_status_string.restype = C.c_char_p
     libetics.etics_status_string.argtypes = [C.c_int]
     assert libetics.etics_status_string(0) == b"ETICS_OK"
-    for code in (-1, -2, -3, -4, -5):
+    for code in (-1, -2, -3, -4, -5, -6):
         assert libetics.etics_status_string(code).startswith(b"ETICS_ERR_")
     assert b"unknown" in libetics.etics_status_string(-99)
 
