@@ -176,6 +176,7 @@ __device__ __forceinline__ void ldcg_words(const unsigned* p, unsigned (&v)[W]) 
     }
 }
 
+template <bool SYNC_AFTER = true>
 __device__ __forceinline__ unsigned block_exclusive_scan_256(unsigned v, unsigned* tmp) {
     // kSortThreads == 256 threads, one value each
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -193,7 +194,7 @@ __device__ __forceinline__ unsigned block_exclusive_scan_256(unsigned v, unsigne
         const unsigned t = tmp[w];
         if (w < warp) woff += t;
     }
-    __syncthreads();
+    if constexpr (SYNC_AFTER) __syncthreads();   // tmp may be rewritten by a caller that does not pass another barrier first
     return woff + inc - v;
 }
 
@@ -364,17 +365,24 @@ __device__ __forceinline__ void sort_phase_scatter(const SortParams& P, SortSmem
             key[i] = (k < N) ? __ldcg(in + k) : ~0ull;   // padding sorts last in every pass and is never written (position >= N)
         }
     };
+    // each warp clears its own counter row (1 << DB 16-bit counters): before the first tile, and again once the row has
+    // been used for the last time in a tile (below) — no block barrier is needed for it
+    auto clear_own_counters = [&]() {
+        uint4* c = reinterpret_cast<uint4*>(&S.cnt[warp][0]);
+        constexpr int kVec = BINS * 2 / 16;
+        static_assert(kVec % 32 == 0, "counter clearing");
+#pragma unroll
+        for (int i = 0; i < kVec / 32; ++i) c[i * 32 + lane] = make_uint4(0u, 0u, 0u, 0u);
+        __syncwarp();
+    };
+    clear_own_counters();
     load_tile(t0);
     for (long long tile = t0; tile < t1; ++tile) {
-        // ---- clear the counters (the tile's words are in registers: loaded while the previous tile was written) ---
-        {
-            uint4* c = reinterpret_cast<uint4*>(&S.cnt[0][0]);
-            constexpr int kVec = kSortWarps * BINS * 2 / 16;
-            static_assert(kVec % kSortThreads == 0, "counter clearing");
-#pragma unroll
-            for (int i = 0; i < kVec / kSortThreads; ++i) c[i * kSortThreads + tid] = make_uint4(0u, 0u, 0u, 0u);
+        // the tile after this one is loaded while this one is written: bring it into L2 now (one 128-byte line per thread)
+        if (tile + 1 < t1) {
+            const long long k = (tile + 1) * kSortTile + (long long)tid * 16;
+            if (k < N) asm volatile("prefetch.global.L2 [%0];" :: "l"(in + k));
         }
-        __syncthreads();
 
         // ---- rank ---------------------------------------------------------------------------------------------
         unsigned short rank[kSortItems];
@@ -408,8 +416,10 @@ __device__ __forceinline__ void sort_phase_scatter(const SortParams& P, SortSmem
             }
         } else {
             // narrow digits: collisions are the rule — the lanes that share a digit find each other with one ballot per digit
-            // bit (register work, independent across the items), then the counters are bumped item by item
-            unsigned peers[kSortItems];
+            // bit; the lowest of them adds the group's size to the warp's counter of that digit (two 16-bit counters per
+            // word: a 32-bit shared-memory atomic, the sums stay below 2^16) and hands the old count to the others.  The atomics
+            // of successive items do not wait for one another's results; __syncwarp orders them (item by item: stable).
+            unsigned* cw32 = reinterpret_cast<unsigned*>(&S.cnt[warp][0]);
 #pragma unroll
             for (int i = 0; i < kSortItems; ++i) {
                 const unsigned d = (unsigned)(key[i] >> dshift) & dmask;
@@ -420,17 +430,13 @@ __device__ __forceinline__ void sort_phase_scatter(const SortParams& P, SortSmem
                     const unsigned vote = __ballot_sync(0xffffffffu, bit);
                     pe &= bit ? vote : ~vote;
                 }
-                peers[i] = pe;
-            }
-#pragma unroll
-            for (int i = 0; i < kSortItems; ++i) {
-                const unsigned d = (unsigned)(key[i] >> dshift) & dmask;
-                const unsigned c = cw[d];
+                const unsigned lower = pe & lt_mask;
+                const unsigned sh = (d & 1u) << 4;
+                unsigned old = 0u;
+                if (lower == 0u) old = atomicAdd(cw32 + (d >> 1), (unsigned)__popc(pe) << sh);
                 __syncwarp();
-                const unsigned lower = peers[i] & lt_mask;
-                rank[i] = (unsigned short)(c + __popc(lower));
-                if (lower == 0u) cw[d] = (unsigned short)(c + __popc(peers[i]));
-                __syncwarp();
+                old = __shfl_sync(0xffffffffu, old, __ffs(pe) - 1);
+                rank[i] = (unsigned short)(((old >> sh) & 0xffffu) + __popc(lower));
             }
         }
         __syncthreads();
@@ -458,7 +464,8 @@ __device__ __forceinline__ void sort_phase_scatter(const SortParams& P, SortSmem
             unsigned run = 0;
 #pragma unroll
             for (int q = 0; q < BPT; ++q) { loc[q] = run; run += tot[q]; }
-            const unsigned off = block_exclusive_scan_256(run, S.scan_tmp);
+            // no barrier after the scan: scan_tmp is not written again before the barriers of the next tile
+            const unsigned off = block_exclusive_scan_256<false>(run, S.scan_tmp);
 #pragma unroll
             for (int q = 0; q < BPT; ++q) loc[q] += off;
             unsigned add[WPT];
@@ -491,6 +498,7 @@ __device__ __forceinline__ void sort_phase_scatter(const SortParams& P, SortSmem
         }
         if (tile + 1 < t1) load_tile(tile + 1);   // in flight while this tile is written
         __syncthreads();
+        clear_own_counters();   // the row was last read by this warp's staging above
 #pragma unroll
         for (int i = 0; i < kSortItems; ++i) {
             const unsigned j = i * kSortThreads + tid;
@@ -499,7 +507,8 @@ __device__ __forceinline__ void sort_phase_scatter(const SortParams& P, SortSmem
             const unsigned g = S.gbase[d] + j;
             if ((long long)g < N) out[g] = kk;
         }
-        __syncthreads();
+        // no block barrier here: stage and gbase are rewritten only after the next tile's barriers, which every thread
+        // reaches after this loop; the counters of the next ranking are this warp's own
     }
 }
 
@@ -557,8 +566,15 @@ __device__ __forceinline__ void sort_phase_fixup(const SortParams& P, const Sort
         for (int j = 0; j < kFixItems; ++j) {
             const long long p = base + j * kSortThreads + threadIdx.x;
             w[j] = (p < N) ? __ldcg(words + p) : 0ull;
-            wl[j] = (p > 0 && p < N) ? __ldcg(words + p - 1) : ~0ull;
-            wr[j] = (p + 1 < N) ? __ldcg(words + p + 1) : ~0ull;
+            // the neighbours are the neighbouring lanes' words; only the warp's edge lanes load theirs
+            wl[j] = (lane == 0 && p > 0 && p < N) ? __ldcg(words + p - 1) : ~0ull;
+            wr[j] = (lane == 31 && p + 1 < N) ? __ldcg(words + p + 1) : ~0ull;
+        }
+#pragma unroll
+        for (int j = 0; j < kFixItems; ++j) {
+            const unsigned long long up = __shfl_up_sync(0xffffffffu, w[j], 1), dn = __shfl_down_sync(0xffffffffu, w[j], 1);
+            if (lane != 0) wl[j] = up;
+            if (lane != 31) wr[j] = dn;
         }
         unsigned long long ks[kFixItems];
         bool lone[kFixItems], head[kFixItems];
