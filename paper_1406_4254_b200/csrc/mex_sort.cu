@@ -556,48 +556,54 @@ __device__ __noinline__ void sort_fix_run(const SortParams& P, const SortPlan& p
 // left free: any order, every head writes a range of its own) for phase F2.
 __device__ __forceinline__ void sort_phase_fixup(const SortParams& P, const SortPlan& pl, const unsigned long long* words,
                                                  unsigned* heads) {
+    // A warp takes kFixItems x 32 consecutive positions per step (item j, lane l: position p0 + 32 j + l).  "Position p and
+    // p + 1 share a prefix" is one comparison per position; everything else — run to the left, alone, head of a run —
+    // follows from the ballots of that bit, in warp-uniform registers.
     const long long N = P.N;
-    const int lane = threadIdx.x & 31;
-    const unsigned long long imask = (1ull << pl.ibits) - 1ull;   // ibits <= 31
-    const long long stride = (long long)gridDim.x * kSortThreads * kFixItems;
-    for (long long base = (long long)blockIdx.x * kSortThreads * kFixItems; base < N; base += stride) {
-        unsigned long long w[kFixItems], wl[kFixItems], wr[kFixItems];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned long long lim = 1ull << pl.ibits;   // same prefix <=> (a ^ b) < lim;  ibits <= 31
+    const unsigned imask = (unsigned)(lim - 1ull);
+    const bool runs = pl.shift > 0;                     // all key bits sorted: no runs at all
+    const unsigned lt_mask = (1u << lane) - 1u;
+    constexpr long long kChunk = 32 * kFixItems;
+    const long long stride = (long long)gridDim.x * kSortWarps * kChunk;
+    for (long long p0 = ((long long)blockIdx.x * kSortWarps + warp) * kChunk; p0 < N; p0 += stride) {
+        unsigned long long w[kFixItems];
 #pragma unroll
         for (int j = 0; j < kFixItems; ++j) {
-            const long long p = base + j * kSortThreads + threadIdx.x;
+            const long long p = p0 + 32 * j + lane;
             w[j] = (p < N) ? __ldcg(words + p) : 0ull;
-            // the neighbours are the neighbouring lanes' words; only the warp's edge lanes load theirs
-            wl[j] = (lane == 0 && p > 0 && p < N) ? __ldcg(words + p - 1) : ~0ull;
-            wr[j] = (lane == 31 && p + 1 < N) ? __ldcg(words + p + 1) : ~0ull;
         }
+        const unsigned long long el = (p0 > 0) ? __ldcg(words + p0 - 1) : 0ull;             // warp-uniform addresses
+        const unsigned long long er = (p0 + kChunk < N) ? __ldcg(words + p0 + kChunk) : 0ull;
+        // R[j]: bit l = the position of (item j, lane l) and the next position share a prefix.  Run to the left, head of a run
+        // and alone follow from R (and c0: the same bit for the position before the chunk) in warp-uniform registers.
+        unsigned R[kFixItems];
+        const unsigned c0 = (runs && p0 > 0 && (((el ^ __shfl_sync(0xffffffffu, w[0], 0)) < lim))) ? 1u : 0u;
 #pragma unroll
         for (int j = 0; j < kFixItems; ++j) {
-            const unsigned long long up = __shfl_up_sync(0xffffffffu, w[j], 1), dn = __shfl_down_sync(0xffffffffu, w[j], 1);
-            if (lane != 0) wl[j] = up;
-            if (lane != 31) wr[j] = dn;
+            const long long p = p0 + 32 * j + lane;
+            // lane l reads the word of lane l + 1; lane 31 reads lane 0's NEXT item (or the word after the chunk)
+            const unsigned long long next0 = (j + 1 < kFixItems) ? w[(j + 1) % kFixItems] : er;
+            const unsigned long long give = (lane == 0) ? next0 : w[j];
+            const unsigned long long nb = __shfl_sync(0xffffffffu, give, (lane + 1) & 31);
+            R[j] = __ballot_sync(0xffffffffu, runs && p + 1 < N && ((w[j] ^ nb) < lim));
         }
-        unsigned long long ks[kFixItems];
-        bool lone[kFixItems], head[kFixItems];
+        auto left = [&](int j) { return (R[j] << 1) | (j > 0 ? R[j > 0 ? j - 1 : 0] >> 31 : c0); };
+        auto valid = [&](int j) {   // lanes whose position is below N
+            const long long n = N - (p0 + 32 * j);
+            return n >= 32 ? 0xffffffffu : n <= 0 ? 0u : (1u << (int)n) - 1u;
+        };
+        unsigned nh = 0;
 #pragma unroll
         for (int j = 0; j < kFixItems; ++j) {
-            const long long p = base + j * kSortThreads + threadIdx.x;
-            const unsigned long long pre = w[j] >> pl.ibits;
-            const bool run_left = pl.shift > 0 && p > 0 && (wl[j] >> pl.ibits) == pre;
-            const bool run_right = pl.shift > 0 && p + 1 < N && (wr[j] >> pl.ibits) == pre;
-            lone[j] = p < N && !run_left && !run_right;
-            head[j] = p < N && !run_left && run_right;
-            ks[j] = (lone[j] && P.keys_sorted) ? __ldcg(P.keys + (unsigned)(w[j] & imask)) : 0ull;
-        }
-        unsigned hm[kFixItems], nh = 0;
-#pragma unroll
-        for (int j = 0; j < kFixItems; ++j) {
-            const long long p = base + j * kSortThreads + threadIdx.x;
-            if (lone[j]) {
-                P.perm[p] = (unsigned)(w[j] & imask);
-                if (P.keys_sorted) P.keys_sorted[p] = ks[j];
+            const bool alone = ((valid(j) & ~R[j] & ~left(j)) >> lane) & 1u;
+            if (alone) {
+                const unsigned idx = (unsigned)w[j] & imask;
+                P.perm[p0 + 32 * j + lane] = idx;
+                if (P.keys_sorted) P.keys_sorted[p0 + 32 * j + lane] = __ldcg(P.keys + idx);   // etics_mex_sort only
             }
-            hm[j] = __ballot_sync(0xffffffffu, head[j]);
-            nh += __popc(hm[j]);
+            nh += __popc(R[j] & ~left(j));
         }
         if (nh) {   // warp-uniform: one atomic per warp and step
             unsigned at = 0;
@@ -605,8 +611,9 @@ __device__ __forceinline__ void sort_phase_fixup(const SortParams& P, const Sort
             at = __shfl_sync(0xffffffffu, at, 0);
 #pragma unroll
             for (int j = 0; j < kFixItems; ++j) {
-                if (head[j]) heads[at + __popc(hm[j] & ((1u << lane) - 1u))] = (unsigned)(base + j * kSortThreads + threadIdx.x);
-                at += __popc(hm[j]);
+                const unsigned H = R[j] & ~left(j);   // heads of runs
+                if ((H >> lane) & 1u) heads[at + __popc(H & lt_mask)] = (unsigned)(p0 + 32 * j + lane);
+                at += __popc(H);
             }
         }
     }
@@ -796,7 +803,7 @@ mex_sort_scatter_kernel(const __grid_constant__ SortParams P, int pass) {
     sort_phase_scatter<kLargeDB>(P, S, pl, pass, (pass & 1) ? P.bufB : P.bufA, (pass & 1) ? P.bufA : P.bufB);
 }
 
-__global__ void __launch_bounds__(kSortThreads)
+__global__ void __launch_bounds__(kSortThreads, 4)
 mex_sort_fixup_kernel(const __grid_constant__ SortParams P) {
     const SortPlan pl = load_plan(P.hdr, P.N, P.prefix_bits, P.digit_bits);
     sort_phase_fixup(P, pl, (pl.passes & 1) ? P.bufB : P.bufA, reinterpret_cast<unsigned*>((pl.passes & 1) ? P.bufA : P.bufB));
