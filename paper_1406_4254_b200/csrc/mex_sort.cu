@@ -359,10 +359,16 @@ __device__ __forceinline__ void sort_phase_scatter(const SortParams& P, SortSmem
     unsigned long long key[kSortItems];
     auto load_tile = [&](long long tile) {
         const long long base = tile * kSortTile + (long long)warp * (32 * kSortItems);
+        const unsigned long long* src = in + base + lane;
+        if ((tile + 1) * kSortTile <= N) {   // every tile but the last one: no bounds checks
 #pragma unroll
-        for (int i = 0; i < kSortItems; ++i) {
-            const long long k = base + 32 * i + lane;
-            key[i] = (k < N) ? __ldcg(in + k) : ~0ull;   // padding sorts last in every pass and is never written (position >= N)
+            for (int i = 0; i < kSortItems; ++i) key[i] = __ldcg(src + 32 * i);
+        } else {
+#pragma unroll
+            for (int i = 0; i < kSortItems; ++i) {
+                const long long k = base + 32 * i + lane;
+                key[i] = (k < N) ? __ldcg(in + k) : ~0ull;   // padding sorts last in every pass and is never written (position >= N)
+            }
         }
     };
     // each warp clears its own counter row (1 << DB 16-bit counters): before the first tile, and again once the row has
