@@ -29,6 +29,7 @@ EXPORTS = [
     "etics_mex_full_host", "etics_mex_force_timed", "etics_probe_dfma", "etics_probe_copy",
     "etics_kernel_launches", "etics_step_host_scratch_bytes", "etics_step_host", "etics_stepper_workspace_bytes", "etics_stepper_create", "etics_stepper_step", "etics_stepper_set_coefficient_interval", "etics_stepper_destroy",
     "etics_scf_coeffs_static_max_table", "etics_scf_coeffs_static",
+    "etics_mex_shard_rows", "etics_mex_shard_moments", "etics_mex_shard_bases", "etics_mex_shard_force",
 ]
 
 _lib = None
@@ -77,6 +78,14 @@ def lib() -> C.CDLL:
     L.etics_mex_force_ex.argtypes = [_vp, _vp, _ll, _i, _i, _vp, _vp, _vp, _sz, _vp]
     L.etics_mex_sort.restype = _i
     L.etics_mex_sort.argtypes = [_vp, _ll, _vp, _vp, _vp, _sz, _vp]
+    L.etics_mex_shard_rows.restype = _i
+    L.etics_mex_shard_rows.argtypes = [_i]
+    L.etics_mex_shard_moments.restype = _i
+    L.etics_mex_shard_moments.argtypes = [_vp, _vp, _ll, _i, _vp, _vp, _sz, _vp]
+    L.etics_mex_shard_bases.restype = _i
+    L.etics_mex_shard_bases.argtypes = [_vp, _i, _i, _i, _vp, _vp]
+    L.etics_mex_shard_force.restype = _i
+    L.etics_mex_shard_force.argtypes = [_ll, _i, _i, _vp, _vp, _vp, _vp, _sz, _vp]
     L.etics_host_scratch_bytes.restype = _sz
     L.etics_host_scratch_bytes.argtypes = [_i, _ll, _i, _i]
     L.etics_scf_full_host.restype = _i
@@ -291,6 +300,46 @@ def etics_mex_sort(pos, keys_sorted=None, perm=None, workspace=None, stream=None
                              _dev(perm, "perm", torch.int32), workspace.data_ptr(), wsb, _stream(stream))
     _check(s, "etics_mex_sort")
     return keys_sorted, perm
+
+
+def etics_mex_shard_rows(lmax: int) -> int:
+    return lib().etics_mex_shard_rows(lmax)
+
+
+def etics_mex_shard_moments(pos, mass, lmax: int, workspace, totals=None, stream=None):
+    """Phase 1 of the radius-partitioned MEX for one shard: -> totals (R,), the shard's moment vector.  `workspace` (a CUDA
+    byte tensor of etics_workspace_bytes(ETICS_WS_MEX_FORCE, N, 0, lmax)) carries the shard's state to etics_mex_shard_force."""
+    N = mass.shape[0]
+    if totals is None:
+        totals = torch.empty(etics_mex_shard_rows(lmax), dtype=torch.float64, device=pos.device)
+    assert pos.shape == (3, N)
+    s = lib().etics_mex_shard_moments(_dev(pos, "pos"), _dev(mass, "mass"), N, lmax, _dev(totals, "totals"),
+                                      workspace.data_ptr(), workspace.numel() * workspace.element_size(), _stream(stream))
+    _check(s, "etics_mex_shard_moments")
+    return totals
+
+
+def etics_mex_shard_bases(parts, rank: int, lmax: int, base=None, stream=None):
+    """parts (nparts, R) CUDA fp64, the shards' moment vectors in radius order -> base (R,) of shard `rank`."""
+    nparts, R = parts.shape
+    assert R == etics_mex_shard_rows(lmax)
+    if base is None:
+        base = torch.empty(R, dtype=torch.float64, device=parts.device)
+    _check(lib().etics_mex_shard_bases(_dev(parts, "parts"), nparts, rank, lmax, _dev(base, "base"), _stream(stream)),
+           "etics_mex_shard_bases")
+    return base
+
+
+def etics_mex_shard_force(N: int, lmax: int, what: int, base, workspace, acc=None, pot=None, stream=None):
+    """Phase 2: scans from `base`, evaluation; acc (3,N), pot (N,) at the shard's local indices."""
+    if acc is None and what != ETICS_WHAT_POTENTIAL:
+        acc = torch.empty((3, N), dtype=torch.float64, device=base.device)
+    if pot is None and what != ETICS_WHAT_FORCE:
+        pot = torch.empty(N, dtype=torch.float64, device=base.device)
+    s = lib().etics_mex_shard_force(N, lmax, what, _dev(base, "base"), _opt(acc, "acc"), _opt(pot, "pot"),
+                                    workspace.data_ptr(), workspace.numel() * workspace.element_size(), _stream(stream))
+    _check(s, "etics_mex_shard_force")
+    return (None if what == ETICS_WHAT_POTENTIAL else acc), (None if what == ETICS_WHAT_FORCE else pot)
 
 
 def etics_host_scratch_bytes(method: int, N: int, nmax: int, lmax: int) -> int:

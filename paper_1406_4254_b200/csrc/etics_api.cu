@@ -129,6 +129,41 @@ etics_status etics_mex_sort(const double* pos, long long N, unsigned long long* 
     return from_cuda(mex_sort_launch(pos, N, keys_sorted, perm, workspace, static_cast<cudaStream_t>(stream)));
 }
 
+// ---- radius-partitioned MEX --------------------------------------------------------------------------------
+int etics_mex_shard_rows(int lmax) {
+    return (lmax < 0 || lmax > ETICS_MAX_LMAX) ? 0 : mex_shard_rows(lmax);
+}
+
+etics_status etics_mex_shard_moments(const double* pos, const double* mass, long long N, int lmax, double* totals,
+                                     void* workspace, size_t workspace_bytes, void* stream) {
+    etics_status s = check_sizes(N, 0, lmax);
+    if (s != ETICS_OK) return s;
+    if (!pos || !mass || !totals || !workspace) return ETICS_ERR_ARG;
+    if (misaligned(pos) || misaligned(mass) || misaligned(totals) || misaligned(workspace)) return ETICS_ERR_ALIGN;
+    if (workspace_bytes < etics_workspace_bytes(ETICS_WS_MEX_FORCE, N, 0, lmax)) return ETICS_ERR_WORKSPACE;
+    return from_cuda(mex_shard_moments_launch(pos, mass, N, lmax, totals, workspace, static_cast<cudaStream_t>(stream)));
+}
+
+etics_status etics_mex_shard_bases(const double* parts, int nparts, int rank, int lmax, double* base, void* stream) {
+    if (lmax < 0 || nparts < 1 || rank < 0 || rank >= nparts || !parts || !base) return ETICS_ERR_ARG;
+    if (lmax > ETICS_MAX_LMAX) return ETICS_ERR_LIMIT;
+    if (misaligned(parts) || misaligned(base)) return ETICS_ERR_ALIGN;
+    return from_cuda(mex_shard_bases_launch(parts, nparts, rank, lmax, base, static_cast<cudaStream_t>(stream)));
+}
+
+etics_status etics_mex_shard_force(long long N, int lmax, int what, const double* base, double* acc, double* pot,
+                                   void* workspace, size_t workspace_bytes, void* stream) {
+    etics_status s = check_sizes(N, 0, lmax);
+    if (s != ETICS_OK) return s;
+    if (what != ETICS_WHAT_BOTH && what != ETICS_WHAT_POTENTIAL && what != ETICS_WHAT_FORCE) return ETICS_ERR_ARG;
+    if (what == ETICS_WHAT_POTENTIAL) acc = nullptr;
+    if (what == ETICS_WHAT_FORCE) pot = nullptr;
+    if (!base || !workspace || (!acc && what != ETICS_WHAT_POTENTIAL) || (!pot && what != ETICS_WHAT_FORCE)) return ETICS_ERR_ARG;
+    if (misaligned(base) || misaligned(acc) || misaligned(pot) || misaligned(workspace)) return ETICS_ERR_ALIGN;
+    if (workspace_bytes < etics_workspace_bytes(ETICS_WS_MEX_FORCE, N, 0, lmax)) return ETICS_ERR_WORKSPACE;
+    return from_cuda(mex_shard_force_launch(N, lmax, what, base, acc, pot, workspace, static_cast<cudaStream_t>(stream)));
+}
+
 // ---- host-buffer entry points ------------------------------------------------------------------------------
 // Scratch layout: pos[3N] | mass[N] | acc[3N] | pot[N] | A[T] | B[T] | workspace, each 256-byte aligned.
 static size_t seg(size_t doubles) { return round_up(doubles * sizeof(double), 256); }

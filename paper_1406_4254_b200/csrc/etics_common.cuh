@@ -215,6 +215,13 @@ cudaError_t mex_force_launch(const double* pos, const double* mass, long long N,
 
 cudaError_t mex_force_timed(const double* pos, const double* mass, long long N, int lmax, double* acc, double* pot,
                             void* ws, cudaStream_t st, float* stage_ms);
+// radius-partitioned MEX: the force sequence cut at the exchange of the shards' moment vectors
+int mex_shard_rows(int lmax);
+cudaError_t mex_shard_moments_launch(const double* pos, const double* mass, long long N, int lmax, double* totals, void* ws,
+                                     cudaStream_t st);
+cudaError_t mex_shard_bases_launch(const double* parts, int nparts, int rank, int lmax, double* base, cudaStream_t st);
+cudaError_t mex_shard_force_launch(long long N, int lmax, int what, const double* base, double* acc, double* pot, void* ws,
+                                   cudaStream_t st);
 
 cudaError_t probe_dfma_launch(int iters, double* sink, double* flops_out, cudaStream_t st);
 cudaError_t probe_copy_launch(void* dst, const void* src, size_t bytes, cudaStream_t st);

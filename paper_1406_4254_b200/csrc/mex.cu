@@ -469,16 +469,17 @@ constexpr int kTileScanThreads = 256;
 constexpr int kTileScanItems = 8;   // consecutive scan-order positions per thread and step
 
 static __global__ void __launch_bounds__(kTileScanThreads)
-mex_tilescan_kernel(double* __restrict__ tot, long long tiles, RowDirs rd) {
+mex_tilescan_kernel(double* __restrict__ tot, long long tiles, RowDirs rd, const double* __restrict__ base) {
     __shared__ double wsum[kTileScanThreads / 32];
     const int row = blockIdx.x, t = threadIdx.x, lane = t & 31, warp = t >> 5;
     bool fwd = true;
     for (int g = 0; g < rd.ng; ++g)
         if (row >= rd.rb[g] && row < rd.rb[g] + 2 * rd.ns[g]) fwd = row < rd.rb[g] + rd.ns[g];
     double* v = tot + (size_t)row * tiles;
-    double carry = 0.0;
-    for (long long base = 0; base < tiles; base += kTileScanThreads * kTileScanItems) {
-        const long long j0 = base + (long long)t * kTileScanItems;   // first scan-order position of this thread
+    // radius-partitioned MEX: the scan starts from the sums of the shards inside (q rows) / outside (p rows) this one
+    double carry = base ? base[row] : 0.0;
+    for (long long b0 = 0; b0 < tiles; b0 += kTileScanThreads * kTileScanItems) {
+        const long long j0 = b0 + (long long)t * kTileScanItems;   // first scan-order position of this thread
         double x[kTileScanItems];
 #pragma unroll
         for (int e = 0; e < kTileScanItems; ++e) {
@@ -516,6 +517,41 @@ mex_tilescan_kernel(double* __restrict__ tot, long long tiles, RowDirs rd) {
         carry += total;
     }
 }
+
+// Radius-partitioned MEX: the sum of every row of the tile totals = this shard's moment
+// vector.  One block per row; thread t adds the tiles t, t + 256, ... in order, then a fixed tree over the threads.
+static __global__ void __launch_bounds__(kTileScanThreads)
+mex_rowtotal_kernel(const double* __restrict__ tot, long long tiles, double* __restrict__ totals) {
+    __shared__ double part[kTileScanThreads];
+    const int row = blockIdx.x, t = threadIdx.x;
+    const double* v = tot + (size_t)row * tiles;
+    double s = 0.0;
+    for (long long j = t; j < tiles; j += kTileScanThreads) s += v[j];
+    part[t] = s;
+    __syncthreads();
+    for (int o = kTileScanThreads / 2; o > 0; o >>= 1) {
+        if (t < o) part[t] += part[t + o];
+        __syncthreads();
+    }
+    if (t == 0) totals[row] = part[0];
+}
+
+#if ETICS_MEX_PART == 0
+// base[row] of shard `rank` from the shards' moment vectors parts[s][row], s in radius order: q rows (inside-out) take the
+// shards inside, added from the innermost outwards; p rows (outside-in) the shards outside, added from the outermost inwards.
+static __global__ void mex_shard_bases_kernel(const double* __restrict__ parts, int nparts, int rank, int rows, RowDirs rd,
+                                              double* __restrict__ base) {
+    const int row = blockIdx.x * blockDim.x + threadIdx.x;
+    if (row >= rows) return;
+    bool fwd = true;
+    for (int g = 0; g < rd.ng; ++g)
+        if (row >= rd.rb[g] && row < rd.rb[g] + 2 * rd.ns[g]) fwd = row < rd.rb[g] + rd.ns[g];
+    double s = 0.0;
+    if (fwd) for (int k = 0; k < rank; ++k) s += parts[(size_t)k * rows + row];
+    else for (int k = nparts - 1; k > rank; --k) s += parts[(size_t)k * rows + row];
+    base[row] = s;
+}
+#endif
 
 // =========================================================================================================
 // M5c + M6 + M7: walk, evaluate, transform, scatter.
@@ -694,21 +730,35 @@ cudaError_t mex_sort_launch(const double* pos, long long N, unsigned long long* 
 
 #endif   // ETICS_MEX_PART == 0
 
+static RowDirs mex_row_dirs(int lmax) {
+    RowDirs rd{};
+    rd.ng = mex_num_groups(lmax);
+    for (int g = 0; g < rd.ng; ++g) { rd.rb[g] = mex_row_base(lmax, g); rd.ns[g] = mex_group_slots(lmax, g); }
+    return rd;
+}
+
+// phase 0: the whole sequence (etics_mex_force).  Radius-partitioned MEX splits it at the one point where the shards
+// exchange: phase 1 = gather + tile totals + the shard's moment vector (totals), phase 2 = tile scan starting from `base`,
+// evaluation, unpack.
 template <int LMAX>
 static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, int what, double* acc, double* pot, cudaStream_t st,
-                                    cudaEvent_t* ev) {
+                                    cudaEvent_t* ev, int phase, const double* base, double* totals) {
     double* rec = reinterpret_cast<double*>(ws + L.off_rec);
     unsigned* idxT = reinterpret_cast<unsigned*>(ws + L.off_idxT);
     double* tot = reinterpret_cast<double*>(ws + L.off_tot);
-    mex_gather_totals_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(
-        reinterpret_cast<const double2*>(ws + L.off_pk), reinterpret_cast<const unsigned*>(ws + L.off_perm), N, L.tiles, rec, idxT, tot);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    if (ev) { cudaEventRecord(ev[3], st); cudaEventRecord(ev[4], st); }
-    RowDirs rd{};
-    rd.ng = mex_num_groups(LMAX);
-    for (int g = 0; g < rd.ng; ++g) { rd.rb[g] = mex_row_base(LMAX, g); rd.ns[g] = mex_group_slots(LMAX, g); }
-    mex_tilescan_kernel<<<mex_total_rows(LMAX), kTileScanThreads, 0, st>>>(tot, L.tiles, rd);
+    cudaError_t e = cudaSuccess;
+    if (phase != 2) {
+        mex_gather_totals_kernel<LMAX><<<(unsigned)L.tiles, kMexThreads, 0, st>>>(
+            reinterpret_cast<const double2*>(ws + L.off_pk), reinterpret_cast<const unsigned*>(ws + L.off_perm), N, L.tiles, rec, idxT, tot);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        if (ev) { cudaEventRecord(ev[3], st); cudaEventRecord(ev[4], st); }
+    }
+    if (phase == 1) {
+        mex_rowtotal_kernel<<<mex_total_rows(LMAX), kTileScanThreads, 0, st>>>(tot, L.tiles, totals);
+        return cudaGetLastError();
+    }
+    mex_tilescan_kernel<<<mex_total_rows(LMAX), kTileScanThreads, 0, st>>>(tot, L.tiles, mex_row_dirs(LMAX), base);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[5], st);
@@ -729,12 +779,13 @@ static cudaError_t mex_scan_enqueue(const MexLayout& L, char* ws, long long N, i
 }
 
 // The scan launch sequence of one lmax range per translation unit.
-#define ETICS_SCAN_ARGS const MexLayout &L, char *ws, long long N, int lmax, int what, double *acc, double *pot, cudaStream_t st, cudaEvent_t *ev
+#define ETICS_SCAN_ARGS const MexLayout &L, char *ws, long long N, int lmax, int what, double *acc, double *pot, cudaStream_t st, cudaEvent_t *ev, \
+                        int phase, const double *base, double *totals
 cudaError_t mex_scan_part0(ETICS_SCAN_ARGS);
 cudaError_t mex_scan_part1(ETICS_SCAN_ARGS);
 cudaError_t mex_scan_part2(ETICS_SCAN_ARGS);
 cudaError_t mex_scan_part3(ETICS_SCAN_ARGS);
-#define ETICS_CASE(LM) case LM: return mex_scan_enqueue<LM>(L, ws, N, what, acc, pot, st, ev);
+#define ETICS_CASE(LM) case LM: return mex_scan_enqueue<LM>(L, ws, N, what, acc, pot, st, ev, phase, base, totals);
 #if ETICS_MEX_PART == 0
 cudaError_t mex_scan_part0(ETICS_SCAN_ARGS) {
     switch (lmax) {
@@ -769,6 +820,13 @@ cudaError_t mex_scan_part3(ETICS_SCAN_ARGS) {
 #if ETICS_MEX_PART == 0
 // ev (optional): 7 events recorded at: start, after keygen, after the radix passes, after gather, after aggregate,
 // after tilescan, after evaluate.
+static cudaError_t mex_scan_dispatch(ETICS_SCAN_ARGS) {
+    if (lmax <= 6) return mex_scan_part0(L, ws, N, lmax, what, acc, pot, st, ev, phase, base, totals);
+    if (lmax <= 8) return mex_scan_part1(L, ws, N, lmax, what, acc, pot, st, ev, phase, base, totals);
+    if (lmax == 9) return mex_scan_part2(L, ws, N, lmax, what, acc, pot, st, ev, phase, base, totals);
+    return mex_scan_part3(L, ws, N, lmax, what, acc, pot, st, ev, phase, base, totals);
+}
+
 static cudaError_t mex_force_enqueue(const double* pos, const double* mass, long long N, int lmax, int what,
                                      double* acc, double* pot, void* wsv, cudaStream_t st, cudaEvent_t* ev) {
     const MexLayout L = make_mex_layout(N, lmax);
@@ -778,10 +836,31 @@ static cudaError_t mex_force_enqueue(const double* pos, const double* mass, long
     cudaError_t e = mex_sort_enqueue(pos, mass, N, L, ws, idxA, nullptr, true, st, ev ? ev[1] : nullptr);
     if (e != cudaSuccess) return e;
     if (ev) cudaEventRecord(ev[2], st);
-    if (lmax <= 6) return mex_scan_part0(L, ws, N, lmax, what, acc, pot, st, ev);
-    if (lmax <= 8) return mex_scan_part1(L, ws, N, lmax, what, acc, pot, st, ev);
-    if (lmax == 9) return mex_scan_part2(L, ws, N, lmax, what, acc, pot, st, ev);
-    return mex_scan_part3(L, ws, N, lmax, what, acc, pot, st, ev);
+    return mex_scan_dispatch(L, ws, N, lmax, what, acc, pot, st, ev, 0, nullptr, nullptr);
+}
+
+// ---- radius-partitioned MEX: the sequence above cut at the exchange of the shards' moment vectors -----------------------
+int mex_shard_rows(int lmax) { return mex_total_rows(lmax); }
+
+cudaError_t mex_shard_moments_launch(const double* pos, const double* mass, long long N, int lmax, double* totals, void* wsv,
+                                     cudaStream_t st) {
+    const MexLayout L = make_mex_layout(N, lmax);
+    char* ws = static_cast<char*>(wsv);
+    cudaError_t e = mex_sort_enqueue(pos, mass, N, L, ws, reinterpret_cast<unsigned*>(ws + L.off_perm), nullptr, true, st, nullptr);
+    if (e != cudaSuccess) return e;
+    return mex_scan_dispatch(L, ws, N, lmax, ETICS_WHAT_BOTH, nullptr, nullptr, st, nullptr, 1, nullptr, totals);
+}
+
+cudaError_t mex_shard_bases_launch(const double* parts, int nparts, int rank, int lmax, double* base, cudaStream_t st) {
+    const int rows = mex_total_rows(lmax);
+    mex_shard_bases_kernel<<<(rows + 127) / 128, 128, 0, st>>>(parts, nparts, rank, rows, mex_row_dirs(lmax), base);
+    return cudaGetLastError();
+}
+
+cudaError_t mex_shard_force_launch(long long N, int lmax, int what, const double* base, double* acc, double* pot, void* wsv,
+                                   cudaStream_t st) {
+    const MexLayout L = make_mex_layout(N, lmax);
+    return mex_scan_dispatch(L, static_cast<char*>(wsv), N, lmax, what, acc, pot, st, nullptr, 2, base, nullptr);
 }
 
 cudaError_t mex_force_launch(const double* pos, const double* mass, long long N, int lmax, int what,

@@ -131,3 +131,79 @@ def test_sharded_scf_exchange_two_ranks(tmp_path):
     for x in res:
         assert x["errA"] < 1e-13 and x["errpot"] < 1e-12
     assert res[0]["digest"] == res[1]["digest"]          # bit-identical tables on both ranks
+
+
+MEX_SHARD_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, os.environ["ETICS_ROOT"])
+import numpy as np
+import torch, torch.distributed as dist
+import oracle
+from paper_1406_4254_b200 import sharded, workloads as W
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+n, lmax = 3001, 4
+pos, mass = W.particles("hernquist", n, seed=7)
+pos = pos.copy(); mass = mass.copy()
+mass *= 1.0 + 0.5 * np.sin(np.arange(n))              # unequal masses: a misrouted row cannot go unnoticed
+# ties ACROSS the index shards: particles of the second half at the radius of particles of the first half (same key bits)
+for j in range(0, 40):
+    pos[:, n // 2 + 5 + 3 * j] = pos[[1, 0, 2], 7 * j] * np.array([-1.0, 1.0, -1.0])
+a, b = sharded.shard_range(n, rank, world)
+acc0, pot0, perm0 = oracle.mex_force(pos, mass, lmax, return_perm=True)     # the whole set on every rank: the expected answer
+checks = {}
+
+# stand-ins for the kernels (no GPU here); what is under test is the partition, the exchange and the return path
+def sort(p):
+    k, pm = oracle.mex_sort(p.numpy())
+    return torch.from_numpy(k.view(np.int64)), torch.from_numpy(pm.astype(np.int32))
+def moments(pos_r, mass_r):
+    nr = mass_r.numel()
+    return torch.tensor([float(nr), float(mass_r.sum())], dtype=torch.float64), (pos_r, mass_r)
+def bases(parts, r):
+    return torch.stack([parts[:r, 0].sum(), parts[r + 1:, 1].sum()])
+def force(state, base):
+    pos_r, mass_r = state[0].numpy(), state[1].numpy()
+    nr, c0 = len(mass_r), int(base[0])
+    _, pr = oracle.mex_sort(pos_r)
+    want = perm0[c0:c0 + nr].astype(np.int64)           # this key range = a slice of the whole set's sorted order ...
+    checks["range_is_slice"] = bool(np.array_equal(pos_r[:, pr], pos[:, want]) and np.array_equal(mass_r[pr], mass[want]))
+    checks["mass_outside"] = bool(np.isclose(float(base[1]), mass[perm0[c0 + nr:].astype(np.int64)].sum(), rtol=1e-12))
+    acc_r = np.empty((3, nr)); pot_r = np.empty(nr)
+    acc_r[:, pr] = acc0[:, want]; pot_r[pr] = pot0[want]   # ... whose answer is known: hand it out in arrival order
+    return torch.from_numpy(acc_r), torch.from_numpy(pot_r)
+
+acc, pot = sharded.mex_force_partitioned(torch.from_numpy(np.ascontiguousarray(pos[:, a:b])), torch.from_numpy(mass[a:b].copy()),
+                                         sort, moments, bases, force)
+print("RESULT " + json.dumps({"rank": rank, **checks,
+      "exact": bool(np.array_equal(acc.numpy(), acc0[:, a:b]) and np.array_equal(pot.numpy(), pot0[a:b]))}), flush=True)
+dist.destroy_process_group()
+"""
+
+
+def test_radius_partition_helpers():
+    import torch
+    from paper_1406_4254_b200 import sharded
+    assert sharded.sample_positions(1, 4) == [0, 0, 0, 0]
+    assert sharded.sample_positions(8, 4) == [1, 3, 5, 7]
+    keys = torch.tensor([1, 2, 2, 3, 5, 8])
+    # equal keys never straddle a splitter: both 2s go to rank 1
+    assert sharded.send_counts(keys, torch.tensor([2, 6])) == [1, 4, 1]
+    assert sharded.send_counts(keys, torch.tensor([], dtype=torch.int64)) == [6]
+    assert sharded.send_counts(keys, torch.tensor([0, 100])) == [0, 6, 0]      # empty ranges are legal
+    assert sharded.choose_splitters(torch.tensor([[1, 5, 9, 13], [2, 6, 10, 14]]), 2).tolist() == [9]
+    assert sharded.choose_splitters(torch.tensor([[3, 1, 2]]), 1).numel() == 0
+
+
+def test_radius_partitioned_mex_exchange_two_ranks(tmp_path):
+    """every rank's key range is a contiguous slice of the whole set's sorted order (ties
+    across the index shards included, in global index order), the interior-count / exterior-mass bases are the sums over the
+    ranks inside / outside, and every particle's result returns to its owner at its original index."""
+    w = tmp_path / "mex_shard_worker.py"
+    w.write_text(MEX_SHARD_WORKER)
+    r = _torchrun([str(w)])
+    assert r.returncode == 0, r.stderr[-2000:]
+    res = sorted((json.loads(m) for m in re.findall(r"RESULT (\{[^{}]*\})", r.stdout)), key=lambda x: x["rank"])
+    assert [x["rank"] for x in res] == [0, 1]
+    for x in res:
+        assert x["range_is_slice"] and x["mass_outside"] and x["exact"]
