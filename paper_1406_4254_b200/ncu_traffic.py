@@ -3,6 +3,7 @@ bench.py reports as `traffic` (profiles/traffic_<workload>.json).
 
     ncu -i prof.ncu-rep --page raw --csv > raw.csv
     python -m paper_1406_4254_b200.ncu_traffic raw.csv <workload> "<the ncu command that made prof.ncu-rep>" > profiles/traffic_<workload>.json
+    python -m paper_1406_4254_b200.ncu_traffic --summary raw.csv <workload>     # key metrics of the first launch of every kernel (text)
 
 The file records a hash of the kernel sources it was captured from (kernel_source_hash below); bench.py reports the
 numbers only while that hash is the one of the sources it runs, so a capture can never outlive the kernels it measured.
@@ -100,7 +101,45 @@ def load(workload: str) -> tuple[dict, str | None]:
     return d.get("kernels", {}), None
 
 
+SUMMARY_METRICS = [
+    "gpu__time_duration.sum", "dram__bytes_read.sum", "dram__bytes_write.sum", "launch__registers_per_thread",
+    "launch__grid_size", "launch__block_size", "launch__occupancy_limit_registers", "launch__occupancy_limit_shared_mem",
+    "sm__warps_active.avg.pct_of_peak_sustained_active", "smsp__inst_executed.sum", "smsp__issue_active.avg.pct_of_peak_sustained_active",
+    "sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active", "smsp__sass_thread_inst_executed_op_dfma_pred_on.sum",
+    "smsp__sass_thread_inst_executed_op_dmul_pred_on.sum", "smsp__sass_thread_inst_executed_op_dadd_pred_on.sum",
+    "l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum",
+]
+STALL = re.compile(r"smsp__average_warps?_issue_stalled_(\w+)_per_issue_active\.ratio")
+
+
+def summary(raw_csv: str, workload: str) -> str:
+    """Key metrics of the FIRST launch of every kernel in the capture, as text (profiles/*_ncu_full_metrics.txt)."""
+    with open(raw_csv) as f:
+        rows = [r for r in csv.reader(l for l in f if not l.startswith("=="))]
+    hdr, units = rows[0], rows[1]
+    col = {h: i for i, h in enumerate(hdr)}
+    seen, out = set(), [f"===== workload {workload} (kernel_source_hash {kernel_source_hash()}) ====="]
+    for r in rows[2:]:
+        name = r[col["Kernel Name"]]
+        if name in seen:
+            continue
+        seen.add(name)
+        out.append("-----")
+        out.append(f"  {'Kernel Name':<80} {name}")
+        for m in SUMMARY_METRICS:
+            if m in col and r[col[m]] not in ("", "n/a"):
+                out.append(f"  {m:<80} {r[col[m]]} {units[col[m]]}")
+        stalls = sorted(((_num(r[i]), STALL.match(h).group(1)) for h, i in col.items() if STALL.match(h) and r[i] not in ("", "n/a")),
+                        reverse=True)[:6]
+        if stalls:
+            out.append("  stalls per issue: " + ", ".join(f"{n} {v:.2f}" for v, n in stalls))
+    return "\n".join(out) + "\n"
+
+
 if __name__ == "__main__":
+    if sys.argv[1] == "--summary":
+        sys.stdout.write(summary(sys.argv[2], sys.argv[3]))
+        sys.exit(0)
     raw, workload, command = sys.argv[1], sys.argv[2], sys.argv[3]
     d = extract(raw)
     d = {"workload": workload, "kernel_source_hash": kernel_source_hash(), "command": command,
