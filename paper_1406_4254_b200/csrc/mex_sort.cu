@@ -12,8 +12,8 @@
 // waits for another block's progress, and everything is integer work in a fixed order.
 //   N <= one tile per resident block (~1.2e6): ONE cooperative kernel, grid-wide barriers between the phases, B = 33,
 //     three 11-bit passes (the sort is a single wave and latency-bound: fewer, wider passes).
-//   larger N: one kernel per phase, B = 36, four 9-bit passes (bandwidth-bound: with 2048 digit values a 4096-word tile
-//     scatters runs of two words; 512 values give 64-byte runs).
+//   larger N: one kernel per phase, B = 36, four 9-bit passes over 5120-word tiles, two scatter blocks per SM (bandwidth-bound:
+//     with 2048 digit values a tile scatters runs of two words; 512 values give 80-byte runs).
 //   mex_sort_fallback_kernel: a run longer than kFixMaxRun (many particles within 2^shift ulps of each other, yet not
 //     all equal: e.g. two thin shells) raises a flag and this plain single-block LSD sort of the full keys redoes the
 //     job — correct for any input, slow, never taken by the paper's workloads.
@@ -103,18 +103,26 @@ struct SortParams {
     unsigned* perm;
     unsigned* itmp;           // second index buffer of the fallback sort
     unsigned long long* keys_sorted;   // may be null
-    long long tiles, tps;     // tiles of kSortTile words; tiles per segment
+    long long tiles, tps;     // tiles of tile_words words; tiles per segment
+    int tile_words;           // kSortThreads x (items per thread of the scatter kernel)
     int nseg;
     int prefix_bits, digit_bits;   // key bits that are radix-sorted; width of a digit (<= kSortDigitBits)
 };
 
-constexpr int kSortItems = 16;
-constexpr int kSortTile = kSortThreads * kSortItems;       // 4096 words
+constexpr int kSortItems = 16;                             // single-wave sort: 4096-word tiles
+constexpr int kSortTile = kSortThreads * kSortItems;
 static_assert(kSortTile == kSortMinTile, "workspace sizing");
+// Bandwidth-bound sort: words per thread and tile.  N = 1e8, whole sort: 16 words with 3 blocks per SM (80 registers) 5.07 ms;
+// with 2 blocks per SM (128 registers, no spills): 16 -> 4.84, 20 -> 4.745, 22 -> 4.74, 24 -> 4.77, 28 -> 4.73 (spills), 32 with
+// one block per SM 5.32.  Fewer resident blocks mean fewer open write frontiers (segments x 512 digit values) in L2 and
+// longer runs of equal digits per tile (20 words x 256 threads / 512 values = 80 bytes).
+constexpr int kLargeItems = 20;
+constexpr int kLargeMinBlocks = 2;
+static_assert(kLargeItems >= kSortItems && kLargeItems * kSortThreads < 65536, "workspace sizing; 16-bit tile positions");
 constexpr int kScanStrip = 8;                              // digit values per strip of the segment scan (one 32-byte sector)
 
 // DB = bits of a digit (compile time: 11 for the single-wave sort, 9 for the bandwidth-bound one).
-template <int DB>
+template <int DB, int ITEMS = kSortItems>
 struct SortSmem {
     static constexpr int BINS = 1 << DB;
     static constexpr int BPT = BINS / kSortThreads;   // thread t owns digits BPT t .. BPT t + BPT - 1 in the offset steps
@@ -124,7 +132,7 @@ struct SortSmem {
     unsigned run[BINS];                     // scatter: next free global position of digit d for this segment; histogram phases: counts
     unsigned scan_tmp[kSortWarps];
     unsigned long long red[2][kSortWarps];
-    unsigned long long stage[kSortTile];    // scatter: the tile in output order; scan: a strip of the segment histograms
+    unsigned long long stage[kSortThreads * ITEMS];    // scatter: the tile in output order; scan: a strip of the segment histograms
 };
 
 template <int W>
@@ -221,9 +229,22 @@ __device__ __forceinline__ void sort_phase_keys(const SortParams& P, unsigned lo
             if (k < N) {
                 const unsigned long long key = mex_key(x[j], y[j], z[j]);
                 P.keys[k] = key;
-                if (P.pk) { P.pk[2 * k] = make_double2(x[j], y[j]); P.pk[2 * k + 1] = make_double2(z[j], mk[j]); }
                 inv = max(inv, ~key);
                 mx = max(mx, key);
+            }
+            // The warp's 32 records are 1024 contiguous bytes: two fully coalesced 16-byte stores per lane (lane l writes the
+            // (x,y) or (z,m) half of the record of lane l / 2, then of lane 16 + l / 2) instead of two stores that each touch
+            // half of 32 sectors (N = 1e8: 4.86 -> 4.77 ms).
+            if (P.pk) {
+                const long long k0 = base + j * kSortThreads + (threadIdx.x & ~31);   // the warp's first particle
+                const bool hi = lane & 1;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int src = 16 * h + (lane >> 1);
+                    const double ax = __shfl_sync(0xffffffffu, x[j], src), ay = __shfl_sync(0xffffffffu, y[j], src);
+                    const double az = __shfl_sync(0xffffffffu, z[j], src), am = __shfl_sync(0xffffffffu, mk[j], src);
+                    if (k0 + src < N) P.pk[2 * (k0 + src) + (hi ? 1 : 0)] = hi ? make_double2(az, am) : make_double2(ax, ay);
+                }
             }
         }
     }
@@ -252,8 +273,8 @@ __device__ __forceinline__ void sort_phase_hist(const SortParams& P, unsigned* h
     const unsigned dmask = (1u << pl.w(pass)) - 1u;
     for (int i = threadIdx.x; i < bins; i += kSortThreads) hist[i] = 0u;
     __syncthreads();
-    const long long k0 = (long long)seg * P.tps * kSortTile;
-    long long k1 = k0 + P.tps * kSortTile;
+    const long long k0 = (long long)seg * P.tps * P.tile_words;
+    long long k1 = k0 + P.tps * P.tile_words;
     if (k1 > P.N) k1 = P.N;
     for (long long base = k0; base < k1; base += kSortThreads * kKeygenItems) {
         unsigned long long w[kKeygenItems];
@@ -328,10 +349,11 @@ __device__ __forceinline__ void sort_phase_scan(const SortParams& P, unsigned* s
 // otherwise the lanes that share a digit find each other with one ballot per digit bit.  (Measured in round 1:
 // MATCH.ANY iterates over the distinct values of a warp, ~230 cycles for random digits; shared-memory atomics do
 // not return ranks in lane order.)
-template <int DB>
-__device__ __forceinline__ void sort_phase_scatter(const SortParams& P, SortSmem<DB>& S, const SortPlan& pl, int pass,
+template <int DB, int ITEMS>
+__device__ __forceinline__ void sort_phase_scatter(const SortParams& P, SortSmem<DB, ITEMS>& S, const SortPlan& pl, int pass,
                                                    const unsigned long long* in, unsigned long long* out) {
-    constexpr int BINS = SortSmem<DB>::BINS, BPT = SortSmem<DB>::BPT, WPT = BPT / 2;
+    constexpr int BINS = SortSmem<DB, ITEMS>::BINS, BPT = SortSmem<DB, ITEMS>::BPT, WPT = BPT / 2;
+    constexpr int kSortItems = ITEMS, kSortTile = kSortThreads * ITEMS;   // (shadow the single-wave constants)
     const int seg = blockIdx.x;
     if (seg >= P.nseg) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -386,8 +408,12 @@ __device__ __forceinline__ void sort_phase_scatter(const SortParams& P, SortSmem
     for (long long tile = t0; tile < t1; ++tile) {
         // the tile after this one is loaded while this one is written: bring it into L2 now (one 128-byte line per thread)
         if (tile + 1 < t1) {
-            const long long k = (tile + 1) * kSortTile + (long long)tid * 16;
-            if (k < N) asm volatile("prefetch.global.L2 [%0];" :: "l"(in + k));
+#pragma unroll
+            for (int h = 0; h < (kSortItems + 15) / 16; ++h) {
+                const int w = (h * kSortThreads + tid) * 16;   // one 128-byte line per thread and round
+                const long long k = (tile + 1) * kSortTile + w;
+                if (w < kSortTile && k < N) asm volatile("prefetch.global.L2 [%0];" :: "l"(in + k));
+            }
         }
 
         // ---- rank ---------------------------------------------------------------------------------------------
@@ -759,7 +785,7 @@ mex_sort_small_kernel(const __grid_constant__ SortParams P) {
         ETICS_PROF();
         grid.sync();
         ETICS_PROF();
-        sort_phase_scatter<kSmallDB>(P, S, pl, pass, in, out);
+        sort_phase_scatter<kSmallDB, kSortItems>(P, S, pl, pass, in, out);
         ETICS_PROF();
         grid.sync();
         ETICS_PROF();
@@ -800,13 +826,15 @@ mex_sort_scan_kernel(const __grid_constant__ SortParams P, int pass) {
     sort_phase_scan(P, strip, 1 << kLargeDB);
 }
 
-__global__ void __launch_bounds__(kSortThreads, 3)
+using LargeSmem = SortSmem<kLargeDB, kLargeItems>;
+
+__global__ void __launch_bounds__(kSortThreads, kLargeMinBlocks)
 mex_sort_scatter_kernel(const __grid_constant__ SortParams P, int pass) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    SortSmem<kLargeDB>& S = *reinterpret_cast<SortSmem<kLargeDB>*>(smem_raw);
+    LargeSmem& S = *reinterpret_cast<LargeSmem*>(smem_raw);
     const SortPlan pl = load_plan(P.hdr, P.N, P.prefix_bits, P.digit_bits);
     if (pass >= pl.passes) return;
-    sort_phase_scatter<kLargeDB>(P, S, pl, pass, (pass & 1) ? P.bufB : P.bufA, (pass & 1) ? P.bufA : P.bufB);
+    sort_phase_scatter<kLargeDB, kLargeItems>(P, S, pl, pass, (pass & 1) ? P.bufB : P.bufA, (pass & 1) ? P.bufA : P.bufB);
 }
 
 __global__ void __launch_bounds__(kSortThreads, 4)
@@ -844,9 +872,9 @@ static cudaError_t sort_device(SortDevice* out) {
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     d.small_blocks = device_sm_count() * per_sm;
     if (d.small_blocks > kSortMaxSegs) d.small_blocks = kSortMaxSegs;
-    e = cudaFuncSetAttribute(mex_sort_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem<kLargeDB>));
+    e = cudaFuncSetAttribute(mex_sort_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LargeSmem));
     if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mex_sort_scatter_kernel, kSortThreads, sizeof(SortSmem<kLargeDB>));
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mex_sort_scatter_kernel, kSortThreads, sizeof(LargeSmem));
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     d.scatter_blocks = device_sm_count() * per_sm;
@@ -887,6 +915,7 @@ cudaError_t mex_sort_enqueue(const double* pos, const double* mass, long long N,
     P.perm = perm_out; P.keys_sorted = keys_sorted_out;
     P.itmp = reinterpret_cast<unsigned*>(ws + L.off_itmp);
     P.tiles = (N + kSortTile - 1) / kSortTile;
+    P.tile_words = kSortTile;
     e = cudaMemsetAsync(ws + L.off_hdr, 0, sizeof(SortHeader), st);
     if (e != cudaSuccess) return e;
     if (P.tiles <= dv.small_blocks) {
@@ -908,7 +937,9 @@ cudaError_t mex_sort_enqueue(const double* pos, const double* mass, long long N,
         // Bandwidth-bound: one kernel per phase, a block per segment of consecutive tiles (two waves of segments), four
         // passes of 9-bit digits over 36 prefix bits — with 2048 digit values a tile of 4096 words would scatter runs of
         // two words (N = 1e8: 1.41 ms per scatter against 0.66 ms), and fewer prefix bits leave more runs to the fix-up.
-        long long segs = 2ll * dv.scatter_blocks;
+        P.tile_words = kSortThreads * kLargeItems;
+        P.tiles = (N + P.tile_words - 1) / P.tile_words;
+        long long segs = 2ll * dv.scatter_blocks;   // two waves of segments (N = 1e8: one wave 4.95 ms, two 4.77, three 4.81)
         if (segs > kSortMaxSegs) segs = kSortMaxSegs;
         P.tps = (P.tiles + segs - 1) / segs;
         P.nseg = (int)((P.tiles + P.tps - 1) / P.tps);
@@ -920,7 +951,7 @@ cudaError_t mex_sort_enqueue(const double* pos, const double* mass, long long N,
         for (int pass = 0; pass < kPasses; ++pass) {
             mex_sort_hist_kernel<<<P.nseg, kSortThreads, 0, st>>>(P, pass);
             mex_sort_scan_kernel<<<(1 << kLargeDB) / kScanStrip, kSortThreads, 0, st>>>(P, pass);
-            mex_sort_scatter_kernel<<<P.nseg, kSortThreads, sizeof(SortSmem<kLargeDB>), st>>>(P, pass);
+            mex_sort_scatter_kernel<<<P.nseg, kSortThreads, sizeof(LargeSmem), st>>>(P, pass);
         }
         mex_sort_fixup_kernel<<<wide, kSortThreads, 0, st>>>(P);
         mex_sort_fixruns_kernel<<<wide, kSortThreads, 0, st>>>(P);

@@ -142,6 +142,14 @@ def test_sort_large_path_collisions_and_fallback(E):
     check_sort(E, pos)
 
 
+@pytest.mark.parametrize("n", [1_279_999, 1_280_000, 1_280_001, 1_515_520 + 4097])
+def test_sort_large_path_tile_boundaries(E, n):
+    """One-kernel-per-phase sort at sizes one below, at and one above a whole number of its 5120-word scatter tiles (250 of
+    them), and one where the last segment holds a single ragged tile."""
+    pos, _ = W.particles("hernquist", n, seed=23)
+    check_sort(E, pos)
+
+
 def test_sort_narrow_range_is_exact_without_fixup(E):
     """A thin shell: the whole key range fits the sorted prefix (shift = 0), whatever N."""
     rng = np.random.default_rng(11)
