@@ -103,8 +103,7 @@ struct SortParams {
     unsigned* perm;
     unsigned* itmp;           // second index buffer of the fallback sort
     unsigned long long* keys_sorted;   // may be null
-    long long tiles, tps;     // tiles of tile_words words; tiles per segment
-    int tile_words;           // kSortThreads x (items per thread of the scatter kernel)
+    long long tiles, tps;     // tiles (kSortTile words in the single-wave sort, kSortThreads * kLargeItems above); tiles per segment
     int nseg;
     int prefix_bits, digit_bits;   // key bits that are radix-sorted; width of a digit (<= kSortDigitBits)
 };
@@ -264,7 +263,8 @@ __device__ __forceinline__ void sort_phase_keys(const SortParams& P, unsigned lo
 }
 
 // phases W (FIRST: words are built from the keys and stored) and H: digit histogram of this block's segment
-template <bool FIRST>
+// TILE: words per tile (a compile-time constant in both kernels that call this)
+template <bool FIRST, int TILE>
 __device__ __forceinline__ void sort_phase_hist(const SortParams& P, unsigned* hist, int bins, const SortPlan& pl, int pass,
                                                 const unsigned long long* in) {
     const int seg = blockIdx.x;
@@ -273,8 +273,8 @@ __device__ __forceinline__ void sort_phase_hist(const SortParams& P, unsigned* h
     const unsigned dmask = (1u << pl.w(pass)) - 1u;
     for (int i = threadIdx.x; i < bins; i += kSortThreads) hist[i] = 0u;
     __syncthreads();
-    const long long k0 = (long long)seg * P.tps * P.tile_words;
-    long long k1 = k0 + P.tps * P.tile_words;
+    const long long k0 = (long long)seg * P.tps * TILE;
+    long long k1 = k0 + P.tps * TILE;
     if (k1 > P.N) k1 = P.N;
     for (long long base = k0; base < k1; base += kSortThreads * kKeygenItems) {
         unsigned long long w[kKeygenItems];
@@ -412,7 +412,7 @@ __device__ __forceinline__ void sort_phase_scatter(const SortParams& P, SortSmem
             for (int h = 0; h < (kSortItems + 15) / 16; ++h) {
                 const int w = (h * kSortThreads + tid) * 16;   // one 128-byte line per thread and round
                 const long long k = (tile + 1) * kSortTile + w;
-                if (w < kSortTile && k < N) asm volatile("prefetch.global.L2 [%0];" :: "l"(in + k));
+                if ((kSortItems % 16 == 0 || w < kSortTile) && k < N) asm volatile("prefetch.global.L2 [%0];" :: "l"(in + k));
             }
         }
 
@@ -768,7 +768,7 @@ mex_sort_small_kernel(const __grid_constant__ SortParams P) {
     grid.sync();
     ETICS_PROF();
     const SortPlan pl = load_plan(P.hdr, P.N, P.prefix_bits, P.digit_bits);
-    sort_phase_hist<true>(P, S.run, BINS, pl, 0, nullptr);
+    sort_phase_hist<true, kSortTile>(P, S.run, BINS, pl, 0, nullptr);
     ETICS_PROF();
     grid.sync();
     ETICS_PROF();
@@ -776,7 +776,7 @@ mex_sort_small_kernel(const __grid_constant__ SortParams P) {
         const unsigned long long* in = (pass & 1) ? P.bufB : P.bufA;
         unsigned long long* out = (pass & 1) ? P.bufA : P.bufB;
         if (pass > 0) {
-            sort_phase_hist<false>(P, S.run, BINS, pl, pass, in);
+            sort_phase_hist<false, kSortTile>(P, S.run, BINS, pl, pass, in);
             ETICS_PROF();
             grid.sync();
             ETICS_PROF();
@@ -814,8 +814,8 @@ mex_sort_hist_kernel(const __grid_constant__ SortParams P, int pass) {
     __shared__ unsigned hist[1 << kLargeDB];
     const SortPlan pl = load_plan(P.hdr, P.N, P.prefix_bits, P.digit_bits);
     if (pass > 0 && pass >= pl.passes) return;
-    if (pass == 0) sort_phase_hist<true>(P, hist, 1 << kLargeDB, pl, 0, nullptr);
-    else sort_phase_hist<false>(P, hist, 1 << kLargeDB, pl, pass, (pass & 1) ? P.bufB : P.bufA);
+    if (pass == 0) sort_phase_hist<true, kSortThreads * kLargeItems>(P, hist, 1 << kLargeDB, pl, 0, nullptr);
+    else sort_phase_hist<false, kSortThreads * kLargeItems>(P, hist, 1 << kLargeDB, pl, pass, (pass & 1) ? P.bufB : P.bufA);
 }
 
 __global__ void __launch_bounds__(kSortThreads)
@@ -915,7 +915,6 @@ cudaError_t mex_sort_enqueue(const double* pos, const double* mass, long long N,
     P.perm = perm_out; P.keys_sorted = keys_sorted_out;
     P.itmp = reinterpret_cast<unsigned*>(ws + L.off_itmp);
     P.tiles = (N + kSortTile - 1) / kSortTile;
-    P.tile_words = kSortTile;
     e = cudaMemsetAsync(ws + L.off_hdr, 0, sizeof(SortHeader), st);
     if (e != cudaSuccess) return e;
     if (P.tiles <= dv.small_blocks) {
@@ -937,8 +936,8 @@ cudaError_t mex_sort_enqueue(const double* pos, const double* mass, long long N,
         // Bandwidth-bound: one kernel per phase, a block per segment of consecutive tiles (two waves of segments), four
         // passes of 9-bit digits over 36 prefix bits — with 2048 digit values a tile of 4096 words would scatter runs of
         // two words (N = 1e8: 1.41 ms per scatter against 0.66 ms), and fewer prefix bits leave more runs to the fix-up.
-        P.tile_words = kSortThreads * kLargeItems;
-        P.tiles = (N + P.tile_words - 1) / P.tile_words;
+        constexpr int kLargeTile = kSortThreads * kLargeItems;
+        P.tiles = (N + kLargeTile - 1) / kLargeTile;
         long long segs = 2ll * dv.scatter_blocks;   // two waves of segments (N = 1e8: one wave 4.95 ms, two 4.77, three 4.81)
         if (segs > kSortMaxSegs) segs = kSortMaxSegs;
         P.tps = (P.tiles + segs - 1) / segs;
