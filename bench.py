@@ -455,6 +455,16 @@ def run_ours(args):
             "potential_only": float(np.mean(timed(lambda: E.etics_mex_force_ex(pos, mass, mex_lmax, E.ETICS_WHAT_POTENTIAL, None, pot2, ws_mex), k_iters, 2))),
             "force_only": float(np.mean(timed(lambda: E.etics_mex_force_ex(pos, mass, mex_lmax, E.ETICS_WHAT_FORCE, acc2, None, ws_mex), k_iters, 2)))}
 
+        # the shard calls of a radius-partitioned multi-GPU run, here with ONE shard holding every particle:
+        # the same kernels as etics_mex_force plus the moment-vector kernels; the exchange between ranks is not in this number
+        R = E.etics_mex_shard_rows(mex_lmax)
+        shard_parts = torch.zeros((1, R), dtype=torch.float64, device="cuda")
+
+        def one_shard():
+            E.etics_mex_shard_moments(pos, mass, mex_lmax, ws_mex, totals=shard_parts[0])
+            E.etics_mex_shard_force(N, mex_lmax, E.ETICS_WHAT_BOTH, E.etics_mex_shard_bases(shard_parts, 0, mex_lmax), ws_mex, acc2, pot2)
+        variants["mex_force_ms"]["one_shard_moments_bases_force"] = float(np.mean(timed(one_shard, k_iters, 2)))
+
     # ---- time-stepping reuse: one leapfrog step with plain launches and as a replayed CUDA graph -----------------
     stepper = {}
     if N <= 10_000_000:
