@@ -496,39 +496,83 @@ scf_accumulate_kernel(const double* __restrict__ pos, const double* __restrict__
             for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
             acc[i][j] = v;
         }
-    double* sOut = smem;   // [2T]: cos table then sin table (entries of other groups stay untouched)
-    __syncthreads();
-    for (int r = 0; r < g.rep; ++r) {
-        if (active && my_rep == r && lane == 0) {
-#pragma unroll
+    if constexpr (FULL) {
+        // Every lane now holds the warp's 44 totals.  Lane L hands on the entries a = L and a = L + 32 (a = i * kAccWMax + j): the
+        // table index is computed once per lane instead of once per entry by lane 0 (ncu source view, N = 1e6: the write-out by
+        // lane 0 — 44 guarded read-modify-writes and 44 stores with their index arithmetic — had 7 % of the kernel's samples).
+        double mine[2] = {0.0, 0.0};
+    #pragma unroll
+        for (int i = 0; i < kAccNCH; ++i)
+    #pragma unroll
+            for (int j = 0; j < kAccWMax; ++j) {
+                const int a = i * kAccWMax + j;
+                if ((a & 31) == lane) mine[a >> 5] = acc[i][j];
+            }
+        int tix[2];
+        bool ok[2];
+    #pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int a = lane + 32 * h;
+            const int i = a / kAccWMax, j = a % kAccWMax;
+            const int n = u.n0 + i, f = u.f0 + j;
+            const int m = (f + 1) >> 1;
+            const bool is_sin = (f > 0) && ((f & 1) == 0);
+            ok[h] = active && a < kAccNCH * kAccWMax && n < pl.n1 && j < u.w;
+            tix[h] = ok[h] ? (is_sin ? pl.T : 0) + n * pl.L + lm_index(u.l, m) : 0;
+        }
+        double* sOut = smem;   // [2T]: cos table then sin table (entries of other groups stay untouched)
+        __syncthreads();
+        for (int r = 0; r < g.rep; ++r) {   // replicas of a unit are added in ascending order
+            if (my_rep == r) {
+    #pragma unroll
+                for (int h = 0; h < 2; ++h)
+                    if (ok[h]) sOut[tix[h]] = (r == 0) ? mine[h] : sOut[tix[h]] + mine[h];
+            }
+            __syncthreads();
+        }
+        if (my_rep == 0) {
+            double* out = partial + (size_t)block * 2 * pl.T;
+    #pragma unroll
+            for (int h = 0; h < 2; ++h)
+                if (ok[h]) out[tix[h]] = sOut[tix[h]];
+        }
+    } else {
+        // multi-group tables (millions of particles per block pass loop: the write-out does not matter; with the compact form
+        // ptxas moved spills into the pass loop of <10,false>: (20,10), N = 1e7, 9.72 -> 9.85 ms)
+        double* sOut = smem;   // [2T]: cos table then sin table (entries of other groups stay untouched)
+        __syncthreads();
+        for (int r = 0; r < g.rep; ++r) {
+            if (active && my_rep == r && lane == 0) {
+    #pragma unroll
+                for (int i = 0; i < kAccNCH; ++i)
+    #pragma unroll
+                    for (int j = 0; j < kAccWMax; ++j) {
+                        const int n = u.n0 + i, f = u.f0 + j;
+                        if (n < pl.n1 && j < u.w) {
+                            const int m = (f + 1) >> 1;
+                            const bool is_sin = (f > 0) && ((f & 1) == 0);
+                            const int t = (is_sin ? pl.T : 0) + n * pl.L + lm_index(u.l, m);
+                            sOut[t] = (r == 0) ? acc[i][j] : sOut[t] + acc[i][j];
+                        }
+                    }
+            }
+            __syncthreads();
+        }
+        if (active && my_rep == 0 && lane == 0) {
+            double* out = partial + (size_t)block * 2 * pl.T;
+    #pragma unroll
             for (int i = 0; i < kAccNCH; ++i)
-#pragma unroll
+    #pragma unroll
                 for (int j = 0; j < kAccWMax; ++j) {
                     const int n = u.n0 + i, f = u.f0 + j;
                     if (n < pl.n1 && j < u.w) {
                         const int m = (f + 1) >> 1;
                         const bool is_sin = (f > 0) && ((f & 1) == 0);
                         const int t = (is_sin ? pl.T : 0) + n * pl.L + lm_index(u.l, m);
-                        sOut[t] = (r == 0) ? acc[i][j] : sOut[t] + acc[i][j];
+                        out[t] = sOut[t];
                     }
                 }
         }
-        __syncthreads();
-    }
-    if (active && my_rep == 0 && lane == 0) {
-        double* out = partial + (size_t)block * 2 * pl.T;
-#pragma unroll
-        for (int i = 0; i < kAccNCH; ++i)
-#pragma unroll
-            for (int j = 0; j < kAccWMax; ++j) {
-                const int n = u.n0 + i, f = u.f0 + j;
-                if (n < pl.n1 && j < u.w) {
-                    const int m = (f + 1) >> 1;
-                    const bool is_sin = (f > 0) && ((f & 1) == 0);
-                    const int t = (is_sin ? pl.T : 0) + n * pl.L + lm_index(u.l, m);
-                    out[t] = sOut[t];
-                }
-            }
     }
 }
 
