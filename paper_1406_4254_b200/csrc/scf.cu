@@ -45,6 +45,10 @@ __host__ __device__ constexpr double leg_gamma_c(int l, int m) {
     return (l >= m + 2) ? double((l + m - 1) * (l - 1 - m)) / double((2 * l - 1) * (2 * l - 3)) : 0.0;
 }
 
+// Scale of table entry (l, n, m): [0] h_lm = leg_scale[l][m], [1] g_n h_lm = geg_scale[l][n] * leg_scale[l][m] (monic Gegenbauer
+// variant).  Written once per device by scf_init_constants, read-only afterwards.
+static __device__ double d_pack_scale[2][kMaxL + 1][kMaxN + 1][kMaxL + 1];
+
 // N1C > 0: nmax + 1 known at compile time (the n loops unroll fully and the compiler schedules across them);
 // N1C = 0: run-time nmax.
 // PO: potential only ("faster since the derivatives ... are not calculated") — no C'_n chain, no
@@ -63,19 +67,25 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
     constexpr int L = num_lm(LMAX);
     const int n1 = N1C > 0 ? N1C : nmax + 1;
     constexpr int kEvalThreads = eval_threads(LMAX);
+    // one-shot blocks: the particle's position is asked for before the table repack, so that the DRAM round trip runs under it
+    const long long k1 = (long long)blockIdx.x * kEvalThreads + threadIdx.x;
+    double x1 = 1.0, y1 = 0.0, z1 = 0.0;
+    if (!eval_persistent(LMAX) && k1 < N) { x1 = pos[k1]; y1 = pos[N + k1]; z1 = pos[2 * N + k1]; }
     for (int g = threadIdx.x; g < n1 * L; g += kEvalThreads) {
         const int n = g / L, j = g - n * L;
         int l = 0;
         while (lm_index(l + 1, 0) <= j) ++l;
         const int m = j - lm_index(l, 0);
         // monic recurrences below: C_n = g_n Q_n, P_lm = h_lm q_lm; the scales ride on the coefficients
-        const double sc = kMonicGeg ? c_basis.geg_scale[l][n] * c_basis.leg_scale[l][m] : c_basis.leg_scale[l][m];
+        // (from a table in GLOBAL memory: the lanes ask for different (l, n, m), and a constant-bank load with 32 different
+        // addresses is replayed 32 times — with c_basis here the repack was 17 % of the kernel's stall samples at N = 1e6)
+        const double sc = d_pack_scale[kMonicGeg ? 1 : 0][l][n][m];
         s_tab[n1 * lm_index(l, 0) + n * (l + 1) + m] = make_double2(A[g] * sc, B[g] * sc);
     }
     __syncthreads();
 
-    auto evaluate = [&](const long long k) {
-    const Geom g = geometry(pos[k], pos[N + k], pos[2 * N + k]);
+    auto evaluate = [&](const long long k, const double px, const double py, const double pz) {
+    const Geom g = geometry(px, py, pz);
 
     // cos(m phi), sin(m phi): parked in lane-private shared-memory columns while the n loops run, so that the
     // 4 (l+1) running sums of a level and the two previous angular rows have the registers to themselves
@@ -202,10 +212,10 @@ scf_eval_kernel(const double* __restrict__ pos, long long N, int nmax,
         // the grid is a few blocks per SM: a block repacks the table once and then takes particles k, k + gridDim.x * threads, ...
         // ((20,10), N = 1e7: 6.08 -> 5.66 ms; at lmax <= 6 the loop costs registers: 138 -> 147 us, so those stay one-shot)
 #pragma unroll 1
-        for (long long k = (long long)blockIdx.x * kEvalThreads + threadIdx.x; k < N; k += (long long)gridDim.x * kEvalThreads) evaluate(k);
+        for (long long k = (long long)blockIdx.x * kEvalThreads + threadIdx.x; k < N; k += (long long)gridDim.x * kEvalThreads)
+            evaluate(k, pos[k], pos[N + k], pos[2 * N + k]);
     } else {
-        const long long k = (long long)blockIdx.x * kEvalThreads + threadIdx.x;
-        if (k < N) evaluate(k);
+        if (k1 < N) evaluate(k1, x1, y1, z1);
     }
 }
 
@@ -794,6 +804,21 @@ cudaError_t scf_init_constants() {
     return once.run([] {
         cudaError_t e = etics_upload_constants_now();
         if (e != cudaSuccess) return e;
+        {
+            BasisConstants* c = new BasisConstants;
+            fill_basis_constants(*c);
+            auto* t = new double[2][kMaxL + 1][kMaxN + 1][kMaxL + 1];
+            for (int l = 0; l <= kMaxL; ++l)
+                for (int n = 0; n <= kMaxN; ++n)
+                    for (int m = 0; m <= kMaxL; ++m) {
+                        t[0][l][n][m] = c->leg_scale[l][m];
+                        t[1][l][n][m] = c->geg_scale[l][n] * c->leg_scale[l][m];
+                    }
+            e = cudaMemcpyToSymbol(d_pack_scale, t, sizeof(double) * 2 * (kMaxL + 1) * (kMaxN + 1) * (kMaxL + 1));
+            delete[] t;
+            delete c;
+            if (e != cudaSuccess) return e;
+        }
         return set_kernel_attributes<kMaxL>();
     });
 }
