@@ -102,3 +102,47 @@ def test_config5_mex_full_size(E, plummer_1e8):
     didx = torch.from_numpy(idx).cuda()
     assert rel_err_scalar(pot[didx].cpu().numpy(), pot0, floor=0.0) <= TOL
     assert rel_err_vector(acc[:, didx].cpu().numpy(), acc0) <= TOL
+
+
+def test_config5_mex_in_four_radius_shards(E, plummer_1e8):
+    """configs[4], MEX half, as the four ranks of a radius-partitioned run would see it: the
+    N = 10^8 particles split into four radius ranges, every range through etics_mex_shard_moments / _bases / _force one after the
+    other on this GPU, sampled particles of every range (its first and last ranks included) against the definition."""
+    pos, mass = plummer_1e8
+    n = len(mass)
+    lmax = 8
+    keys0, perm0 = oracle.mex_sort(pos)
+    edges = [0]
+    for c in (n // 4, n // 2 + 12_345, 3 * (n // 4)):
+        while keys0[c] == keys0[c - 1]:      # equal keys stay in one shard
+            c += 1
+        edges.append(c)
+    edges.append(n)
+    R = E.etics_mex_shard_rows(lmax)
+    parts = torch.zeros((4, R), dtype=torch.float64, device="cuda")
+    shards, state = [], []
+    for s in range(4):
+        idx = np.sort(perm0[edges[s]:edges[s + 1]].astype(np.int64))     # a shard keeps the order of the particles' indices
+        ws = torch.empty(E.etics_workspace_bytes(E.ETICS_WS_MEX_FORCE, len(idx), 0, lmax), dtype=torch.uint8, device="cuda")
+        E.etics_mex_shard_moments(torch.from_numpy(np.ascontiguousarray(pos[:, idx])).cuda(), torch.from_numpy(mass[idx]).cuda(),
+                                  lmax, ws, totals=parts[s])
+        shards.append(idx)
+        state.append(ws)
+    torch.cuda.synchronize()
+    got_idx, got_acc, got_pot = [], [], []
+    for s in range(4):
+        idx = shards[s]
+        acc, pot = E.etics_mex_shard_force(len(idx), lmax, E.ETICS_WHAT_BOTH, E.etics_mex_shard_bases(parts, s, lmax), state[s])
+        torch.cuda.synchronize()
+        assert bool(torch.isfinite(acc).all()) and bool(torch.isfinite(pot).all())
+        # samples of this range: its innermost and outermost particles and a few in between (global indices)
+        ranks = np.unique(np.concatenate([np.arange(edges[s], edges[s] + 2), np.arange(edges[s + 1] - 2, edges[s + 1]),
+                                          np.linspace(edges[s], edges[s + 1] - 1, 5).astype(np.int64)]))
+        g = perm0[ranks].astype(np.int64)
+        loc = torch.from_numpy(np.searchsorted(idx, g)).cuda()
+        got_idx.append(g); got_acc.append(acc[:, loc].cpu().numpy()); got_pot.append(pot[loc].cpu().numpy())
+        state[s] = None
+    g = np.concatenate(got_idx)
+    acc0, pot0 = oracle.mex_force_at(pos, mass, lmax, g)
+    assert rel_err_scalar(np.concatenate(got_pot), pot0, floor=0.0) <= TOL
+    assert rel_err_vector(np.concatenate(got_acc, axis=1), acc0) <= TOL
